@@ -1,0 +1,591 @@
+/* noit_oracle.c -- plain, slow, obviously-correct CPU oracle for the neural-OIT resolve.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * `--impl reference` legs may build, load or call this file.  It shares no code, header, table
+ * or helper with the CUDA path (paper_2606_16747_b200/csrc/, include/noit.h) and never calls it.
+ *
+ * Written from /root/reference/PAPER.md ("P:n" = line n of that file) under the readings of
+ * SURVEY.md section 8(c) (O1..O9, A1..A24), restated in DESIGN.md.  The method is an
+ * approximation (a learned tail colour), so this is the algorithm step by step in the paper's
+ * order and notation, not an "exact composite".  Every sum / product whose GPU counterpart is
+ * an fp32 reduction is carried in double here; every DECISION that must be bit-exact (layer
+ * selection, quadtree split, reprojection accept) is taken in the precision the readings fix
+ * (fp32 compare + integer index; exact integers; fp32 in a fixed operation order).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC noit_oracle.c -lm
+ * (-ffp-contract=off: nothing fuses unless written as fmaf).  OpenMP only parallelises the
+ * outer pixel / tile loops; every pixel is computed by the same scalar code.
+ *
+ * Pins (tests/test_oracle_*.py): brute-force sort, empty-tail identity, exact-tail identity,
+ * closed forms, numpy float64 MLP, quadtree closed forms + big-int brute force, reprojection
+ * identity / integer shift.  PARITY UNPINNED: agreement of features O3 (reading A1), of the
+ * corner metric's constant and of any threshold with the authors' shader / supplemental
+ * material / trained weights -- none of those is available.
+ */
+#include <math.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ABSENT 0xFFFFFFFFu
+
+/* ---------------------------------------------------------------------------------------- */
+/* fragment access                                                                           */
+/* ---------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t width, height;
+    const uint32_t *offsets; /* [P+1] */
+    const float *depth;      /* [F]   */
+    const void *rgba;        /* [F][4] _Float16 (fmt 0) or float (fmt 1), straight colour, .w=alpha */
+    int32_t color_fmt;
+} frag_view;
+
+/* fp16 inputs are widened exactly (O2). */
+static void frag_rgba(const frag_view *fb, uint32_t j, double out[4])
+{
+    if (fb->color_fmt == 0) {
+        const _Float16 *h = (const _Float16 *)fb->rgba + 4 * (size_t)j;
+        for (int k = 0; k < 4; ++k) out[k] = (double)(float)h[k];
+    } else {
+        const float *f = (const float *)fb->rgba + 4 * (size_t)j;
+        for (int k = 0; k < 4; ++k) out[k] = (double)f[k];
+    }
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O1 selection + O2 tail accumulators of ONE pixel                                          */
+/* ---------------------------------------------------------------------------------------- */
+typedef struct {
+    uint32_t n;          /* N = n_p */
+    uint32_t i1, i2;     /* GLOBAL fragment indices, ABSENT if missing       */
+    double c1[4], c2[4]; /* straight RGBA of layers 1, 2 (zeros if absent)   */
+    float d1;            /* depth of layer 1, 1.0f if the pixel is empty     */
+    double c_acc[3];     /* C_acc = sum_{tail} alpha_i C_i */
+    double a_tail;       /* sum_{tail} alpha_i                (reading A1)   */
+    double t_tail;       /* prod_{tail} (1 - alpha_i)         (reading A1)   */
+} pixel_layers;
+
+/* key order: fp32 '<' on depth, then integer '<' on the fragment index (O1; tie rule from
+ * BASELINE.json north_star "ties broken by fragment index").  Smaller depth = nearer (A9). */
+static int key_less(float da, uint32_t ia, float db, uint32_t ib)
+{
+    if (da < db) return 1;
+    if (db < da) return 0;
+    return ia < ib;
+}
+
+static void pixel_select_reduce(const frag_view *fb, size_t p, pixel_layers *L)
+{
+    uint32_t b = fb->offsets[p], e = fb->offsets[p + 1];
+    memset(L, 0, sizeof *L);
+    L->n = e - b;
+    L->i1 = L->i2 = ABSENT;
+    L->d1 = 1.0f;
+    L->t_tail = 1.0;
+    /* O1: i1 = smallest key; i2 = smallest key among the rest.  Two plain scans. (P:55, P:95:
+     * "the first two passes compute the first and the second closest fragments")            */
+    for (uint32_t j = b; j < e; ++j)
+        if (L->i1 == ABSENT || key_less(fb->depth[j], j, fb->depth[L->i1], L->i1)) L->i1 = j;
+    for (uint32_t j = b; j < e; ++j) {
+        if (j == L->i1) continue;
+        if (L->i2 == ABSENT || key_less(fb->depth[j], j, fb->depth[L->i2], L->i2)) L->i2 = j;
+    }
+    if (L->i1 != ABSENT) { frag_rgba(fb, L->i1, L->c1); L->d1 = fb->depth[L->i1]; }
+    if (L->i2 != ABSENT) frag_rgba(fb, L->i2, L->c2);
+    /* O2: third pass -- every fragment that is not one of the two peeled layers, in index
+     * order (P:117 C_acc = sum_{i=3}^{N} alpha_i C_i; P:111 prod (1 - a_i)).                 */
+    for (uint32_t j = b; j < e; ++j) {
+        if (j == L->i1 || j == L->i2) continue;
+        double c[4];
+        frag_rgba(fb, j, c);
+        for (int k = 0; k < 3; ++k) L->c_acc[k] += c[3] * c[k];
+        L->a_tail += c[3];
+        L->t_tail *= (1.0 - c[3]);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O3 features                                                                               */
+/* ---------------------------------------------------------------------------------------- */
+/* x = [N, t_tail, C_acc / a_tail]  (readings A1, A2, A5); rounded to fp32 once.   */
+static int features_from(double n, double t_tail, const double c_acc[3], double a_tail, float x[5])
+{
+    int has_tail = a_tail > 0.0;
+    x[0] = (float)n;
+    x[1] = (float)t_tail;
+    for (int k = 0; k < 3; ++k) x[2 + k] = has_tail ? (float)(c_acc[k] / a_tail) : 0.0f;
+    return has_tail;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O4 MLP 5 -> 32 -> 16 -> 3, ReLU on both hidden layers (A3) and on the output        */
+/* ---------------------------------------------------------------------------------------- */
+/* w: 771 EFFECTIVE weights W1[32][5], b1[32], W2[16][32], b2[16], W3[3][16], b3[3] (row =
+ * output neuron).  Each dot product is accumulated in double, in input-index order, starting
+ * from the bias.  Activations are never rounded (A6).                                        */
+static void mlp_forward(const float *w, const float x[5], double f[3])
+{
+    const float *W1 = w, *b1 = W1 + 32 * 5, *W2 = b1 + 32, *b2 = W2 + 16 * 32;
+    const float *W3 = b2 + 16, *b3 = W3 + 3 * 16;
+    double h1[32], h2[16];
+    for (int o = 0; o < 32; ++o) {
+        double a = (double)b1[o];
+        for (int i = 0; i < 5; ++i) a += (double)W1[o * 5 + i] * (double)x[i];
+        h1[o] = a > 0.0 ? a : 0.0;
+    }
+    for (int o = 0; o < 16; ++o) {
+        double a = (double)b2[o];
+        for (int i = 0; i < 32; ++i) a += (double)W2[o * 32 + i] * h1[i];
+        h2[o] = a > 0.0 ? a : 0.0;
+    }
+    for (int o = 0; o < 3; ++o) {
+        double a = (double)b3[o];
+        for (int i = 0; i < 16; ++i) a += (double)W3[o * 16 + i] * h2[i];
+        f[o] = a > 0.0 ? a : 0.0;
+    }
+}
+
+/* bf16 weight mode (A6): each weight rounded to bf16, round-to-nearest-even, then widened.   */
+void oracle_round_weights_bf16(float *w, int32_t count)
+{
+    for (int32_t i = 0; i < count; ++i) {
+        uint32_t u;
+        memcpy(&u, &w[i], 4);
+        if ((u & 0x7F800000u) != 0x7F800000u) {           /* finite */
+            uint32_t lsb = (u >> 16) & 1u;
+            u += 0x7FFFu + lsb;
+        }
+        u &= 0xFFFF0000u;
+        memcpy(&w[i], &u, 4);
+    }
+}
+
+int32_t oracle_infer(const float *weights, const float *features, uint32_t n, float *tail_rgb)
+{
+    if (!weights || !features || !tail_rgb) return 1;
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < (int64_t)n; ++r) {
+        double f[3];
+        mlp_forward(weights, features + 5 * r, f);
+        for (int k = 0; k < 3; ++k) tail_rgb[3 * r + k] = (float)f[k];
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* S1-S3: layers, tail accumulators, features for every pixel                                */
+/* ---------------------------------------------------------------------------------------- */
+/* Any output may be NULL.  idx1/idx2 are LOCAL indices (j - offsets[p]), ABSENT if missing.  */
+int32_t oracle_build_features(int32_t width, int32_t height, const uint32_t *offsets,
+                              const float *depth, const void *rgba, int32_t color_fmt,
+                              uint32_t *idx1, uint32_t *idx2, uint32_t *count, float *layer1,
+                              float *layer2, float *depth1, float *tail_raw, float *features)
+{
+    frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
+    int64_t P = (int64_t)width * height;
+#pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t p = 0; p < P; ++p) {
+        pixel_layers L;
+        pixel_select_reduce(&fb, (size_t)p, &L);
+        if (idx1) idx1[p] = L.i1 == ABSENT ? ABSENT : L.i1 - offsets[p];
+        if (idx2) idx2[p] = L.i2 == ABSENT ? ABSENT : L.i2 - offsets[p];
+        if (count) count[p] = L.n;
+        if (layer1) for (int k = 0; k < 4; ++k) layer1[4 * p + k] = (float)L.c1[k];
+        if (layer2) for (int k = 0; k < 4; ++k) layer2[4 * p + k] = (float)L.c2[k];
+        if (depth1) depth1[p] = L.d1;
+        if (tail_raw) {
+            for (int k = 0; k < 3; ++k) tail_raw[5 * p + k] = (float)L.c_acc[k];
+            tail_raw[5 * p + 3] = (float)L.a_tail;
+            tail_raw[5 * p + 4] = (float)L.t_tail;
+        }
+        if (features) features_from((double)L.n, L.t_tail, L.c_acc, L.a_tail, features + 5 * p);
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O5 composite (Eq. 4) and O7 adaptive variant                                    */
+/* ---------------------------------------------------------------------------------------- */
+static void store_outputs(int64_t p, const double ct[3], double t_tot, const float bg[3], float d1,
+                          float *out_trans, float *out_final, float *out_depth1)
+{
+    if (out_trans) {
+        for (int k = 0; k < 3; ++k) out_trans[4 * p + k] = (float)ct[k];
+        out_trans[4 * p + 3] = (float)t_tot;
+    }
+    if (out_final) {                 /* C_p = C_t + prod(1-a_i) C_b  (Eq. 3, Eq. 4)     */
+        for (int k = 0; k < 3; ++k) out_final[4 * p + k] = (float)(ct[k] + t_tot * (double)bg[k]);
+        out_final[4 * p + 3] = (float)(1.0 - t_tot);
+    }
+    if (out_depth1) out_depth1[p] = d1;
+}
+
+/* Plain pixel (lod 0): O1-O5.  tail_override (oracle-only test hook): if non-NULL, f(x) is
+ * replaced by tail_override[p] so that Eq. 4's structure can be pinned without any weights.  */
+static void resolve_pixel_full(const frag_view *fb, int64_t p, const float *weights,
+                               const float *tail_override, const float bg[3], float *out_trans,
+                               float *out_final, float *out_depth1)
+{
+    pixel_layers L;
+    float x[5];
+    double f[3], ct[3];
+    pixel_select_reduce(fb, (size_t)p, &L);
+    int has_tail = features_from((double)L.n, L.t_tail, L.c_acc, L.a_tail, x);
+    if (tail_override) for (int k = 0; k < 3; ++k) f[k] = (double)tail_override[3 * p + k];
+    else mlp_forward(weights, x, f);
+    double a1 = L.c1[3], a2 = L.c2[3];           /* absent layers have alpha = 0 (A10)        */
+    double t2 = (1.0 - a1) * (1.0 - a2);         /* T_2                               */
+    for (int k = 0; k < 3; ++k) {
+        double c_ex = a1 * L.c1[k] + (1.0 - a1) * a2 * L.c2[k];      /* C_exact,2     */
+        ct[k] = c_ex + (has_tail ? t2 * f[k] : 0.0);                 /* A2: no tail, no term  */
+    }
+    store_outputs(p, ct, t2 * L.t_tail, bg, L.d1, out_trans, out_final, out_depth1);
+}
+
+/* G = [a2*C2 (3), a2, C_acc (3), A_tail, T_tail, N] of ONE coarse pixel, self-contained
+ * O1-O2 on the coarse buffer (O7, A19: each coarse pixel peels its own top-2).               */
+static void coarse_G(const frag_view *cb, int cx, int cy, double G[10])
+{
+    pixel_layers L;
+    pixel_select_reduce(cb, (size_t)cy * cb->width + cx, &L);
+    for (int k = 0; k < 3; ++k) G[k] = L.c2[3] * L.c2[k];
+    G[3] = L.c2[3];
+    for (int k = 0; k < 3; ++k) G[4 + k] = L.c_acc[k];
+    G[7] = L.a_tail;
+    G[8] = L.t_tail;
+    G[9] = (double)L.n;
+}
+
+static int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+/* lod > 0 pixel (O7; P:76 pass 1 always full-res; P:87 bilinear upsample of passes 2/3, then
+ * inference and composite at full resolution).  r = 2^lod; leaf_side = 64 >> level.          */
+static void resolve_pixel_coarse(const frag_view *fb, const frag_view *cb, int r, int leaf_side,
+                                 int x, int y, const float *weights, const float bg[3],
+                                 float *out_trans, float *out_final, float *out_depth1)
+{
+    int64_t p = (int64_t)y * fb->width + x;
+    pixel_layers L;
+    pixel_select_reduce(fb, (size_t)p, &L);      /* only layer 1 of it is used                */
+    /* sample position in coarse texel units; taps clamped to the leaf and to the image       */
+    double u = (x + 0.5) / r - 0.5, v = (y + 0.5) / r - 0.5;
+    int i0 = (int)floor(u), j0 = (int)floor(v);
+    double wx = u - i0, wy = v - j0;
+    int lx0 = (x / leaf_side) * leaf_side, ly0 = (y / leaf_side) * leaf_side;
+    int tx_lo = lx0 / r, tx_hi = (lx0 + leaf_side - 1) / r;
+    int ty_lo = ly0 / r, ty_hi = (ly0 + leaf_side - 1) / r;
+    if (tx_hi > cb->width - 1) tx_hi = cb->width - 1;
+    if (ty_hi > cb->height - 1) ty_hi = cb->height - 1;
+    int xa = clampi(i0, tx_lo, tx_hi), xb = clampi(i0 + 1, tx_lo, tx_hi);
+    int ya = clampi(j0, ty_lo, ty_hi), yb = clampi(j0 + 1, ty_lo, ty_hi);
+    double g00[10], g10[10], g01[10], g11[10], G[10];
+    coarse_G(cb, xa, ya, g00);
+    coarse_G(cb, xb, ya, g10);
+    coarse_G(cb, xa, yb, g01);
+    coarse_G(cb, xb, yb, g11);
+    for (int k = 0; k < 10; ++k) {               /* lerp x first, then y                      */
+        double top = g00[k] + wx * (g10[k] - g00[k]);
+        double bot = g01[k] + wx * (g11[k] - g01[k]);
+        G[k] = top + wy * (bot - top);
+    }
+    float xf[5];
+    double f[3], ct[3];
+    int has_tail = features_from(G[9], G[8], &G[4], G[7], xf);
+    mlp_forward(weights, xf, f);
+    double a1 = L.c1[3];
+    double t2 = (1.0 - a1) * (1.0 - G[3]);
+    for (int k = 0; k < 3; ++k)
+        ct[k] = a1 * L.c1[k] + (1.0 - a1) * G[k] + (has_tail ? t2 * f[k] : 0.0);
+    store_outputs(p, ct, t2 * G[8], bg, L.d1, out_trans, out_final, out_depth1);
+}
+
+/* S1-S5 (+S7 when cell_level != NULL, +S9 when pixel_list != NULL).
+ * half/quarter buffers: pass width 0 to mark a buffer as absent.
+ * cell_level[cy*ceil(W/8)+cx] in 0..3 ; level_to_lod[4] in {0,1,2}.
+ * pixel_list/pixel_count: resolve exactly those pixels, leave the rest untouched (O9).       */
+int32_t oracle_resolve(int32_t width, int32_t height, const uint32_t *offsets, const float *depth,
+                       const void *rgba, int32_t color_fmt,
+                       int32_t hw, int32_t hh, const uint32_t *hoff, const float *hdepth,
+                       const void *hrgba,
+                       int32_t qw, int32_t qh, const uint32_t *qoff, const float *qdepth,
+                       const void *qrgba,
+                       const uint8_t *cell_level, const uint8_t *level_to_lod,
+                       const float *weights, const float *tail_override, const float *background,
+                       const uint32_t *pixel_list, uint32_t pixel_count,
+                       float *out_trans, float *out_final, float *out_depth1)
+{
+    frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
+    frag_view hb = {hw, hh, hoff, hdepth, hrgba, color_fmt};
+    frag_view qb = {qw, qh, qoff, qdepth, qrgba, color_fmt};
+    if (!weights && !tail_override) return 4;
+    int64_t P = (int64_t)width * height;
+    int64_t count = pixel_list ? (int64_t)pixel_count : P;
+    int cells_x = (width + 7) / 8;
+#pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t t = 0; t < count; ++t) {
+        int64_t p = pixel_list ? (int64_t)pixel_list[t] : t;
+        int x = (int)(p % width), y = (int)(p / width);
+        int lod = 0, level = 3;
+        if (cell_level) {
+            level = cell_level[(y / 8) * cells_x + (x / 8)];
+            lod = level_to_lod[level];
+        }
+        if (lod == 0)
+            resolve_pixel_full(&fb, p, weights, tail_override, background, out_trans, out_final,
+                               out_depth1);
+        else
+            resolve_pixel_coarse(&fb, lod == 1 ? &hb : &qb, 1 << lod, 64 >> level, x, y, weights,
+                                 background, out_trans, out_final, out_depth1);
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O5x exact reference: sort every fragment (O1 order), then Eq. 1 read with            */
+/* premultiplied C_p = alpha_p * C_p (A8) plus the background term of Eq. 3.           */
+/* Used by the invariants only.                                                              */
+/* ---------------------------------------------------------------------------------------- */
+typedef struct { float d; uint32_t j; } sort_key;
+static int cmp_key(const void *a, const void *b)
+{
+    const sort_key *ka = a, *kb = b;
+    if (key_less(ka->d, ka->j, kb->d, kb->j)) return -1;
+    if (key_less(kb->d, kb->j, ka->d, ka->j)) return 1;
+    return 0;
+}
+
+/* out_final[P][4] = (C, 1 - T);  out_tail[P][3] (optional) = exact composite of the sorted
+ * fragments from the 3rd on, sum_{k>=3} a_k C_k prod_{3<=q<k}(1-a_q), i.e. what f(x) stands for */
+int32_t oracle_exact(int32_t width, int32_t height, const uint32_t *offsets, const float *depth,
+                     const void *rgba, int32_t color_fmt, const float *background,
+                     float *out_final, float *out_tail)
+{
+    frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
+    int64_t P = (int64_t)width * height;
+#pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t p = 0; p < P; ++p) {
+        uint32_t b = offsets[p], e = offsets[p + 1], n = e - b;
+        sort_key *keys = malloc(sizeof(sort_key) * (n ? n : 1));
+        for (uint32_t j = b; j < e; ++j) { keys[j - b].d = depth[j]; keys[j - b].j = j; }
+        qsort(keys, n, sizeof(sort_key), cmp_key);   /* keys are distinct: order is total     */
+        double C[3] = {0, 0, 0}, T = 1.0, Ct[3] = {0, 0, 0}, Tt = 1.0;
+        for (uint32_t k = 0; k < n; ++k) {
+            double c[4];
+            frag_rgba(&fb, keys[k].j, c);
+            for (int ch = 0; ch < 3; ++ch) C[ch] += T * c[3] * c[ch];
+            T *= (1.0 - c[3]);
+            if (k >= 2) {
+                for (int ch = 0; ch < 3; ++ch) Ct[ch] += Tt * c[3] * c[ch];
+                Tt *= (1.0 - c[3]);
+            }
+        }
+        free(keys);
+        if (out_final) {
+            for (int ch = 0; ch < 3; ++ch)
+                out_final[4 * p + ch] = (float)(C[ch] + T * (double)background[ch]);
+            out_final[4 * p + 3] = (float)(1.0 - T);
+        }
+        if (out_tail) for (int ch = 0; ch < 3; ++ch) out_tail[3 * p + ch] = (float)Ct[ch];
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O6 quadtree (section 3.1; sizes 64 -> 8 from BASELINE.json cfg4, reading A13)       */
+/* ---------------------------------------------------------------------------------------- */
+typedef struct {
+    const float *image; /* [P][4] */
+    int32_t width, height;
+    int32_t metric;     /* 0 = integer colour variance (primary, A14/A16), 1 = corner D_i    */
+    uint32_t var_threshold_q;
+    float corner_threshold;
+} qt_args;
+
+/* 8-bit quantise: q = rint(255 * clamp(c, 0, 1)), single fp32 multiply, round-half-even.      */
+static uint32_t quant8(float c)
+{
+    float cl = c < 0.0f ? 0.0f : (c > 1.0f ? 1.0f : c);
+    return (uint32_t)lrintf(255.0f * cl);
+}
+
+/* does the node [x0,x0+side) x [y0,y0+side) split?  (strict '>' against the threshold)        */
+static int node_splits(const qt_args *a, int x0, int y0, int side)
+{
+    int x1 = x0 + side, y1 = y0 + side;
+    if (x1 > a->width) x1 = a->width;
+    if (y1 > a->height) y1 = a->height;
+    if (x0 >= x1 || y0 >= y1) return 0;            /* wholly outside the image (A17)         */
+    if (a->metric == 0) {
+        uint64_t n = 0, s1[3] = {0, 0, 0}, s2[3] = {0, 0, 0};
+        for (int y = y0; y < y1; ++y)
+            for (int x = x0; x < x1; ++x) {
+                const float *px = a->image + 4 * ((size_t)y * a->width + x);
+                for (int c = 0; c < 3; ++c) {
+                    uint64_t q = quant8(px[c]);
+                    s1[c] += q;
+                    s2[c] += q * q;
+                }
+                ++n;
+            }
+        /* sum_c (n*S2_c - S1_c^2) > thr * n^2   <=>   sum_c var_c > thr   (8-bit units^2)    */
+        uint64_t lhs = 0;
+        for (int c = 0; c < 3; ++c) lhs += n * s2[c] - s1[c] * s1[c];
+        return lhs > (uint64_t)a->var_threshold_q * n * n;
+    }
+    /* corner metric D_i: mean pairwise Euclidean colour distance of the 4 corner
+     * samples of the node's in-image rectangle; fp32, fixed order (A14)                      */
+    int xs[4] = {x0, x1 - 1, x0, x1 - 1}, ys[4] = {y0, y0, y1 - 1, y1 - 1};
+    static const int pa[6] = {0, 0, 0, 1, 1, 2}, pb[6] = {1, 2, 3, 2, 3, 3};
+    float sum = 0.0f;
+    for (int k = 0; k < 6; ++k) {
+        const float *A = a->image + 4 * ((size_t)ys[pa[k]] * a->width + xs[pa[k]]);
+        const float *B = a->image + 4 * ((size_t)ys[pb[k]] * a->width + xs[pb[k]]);
+        float dr = A[0] - B[0], dg = A[1] - B[1], db = A[2] - B[2];
+        float s = dr * dr;
+        s = s + dg * dg;
+        s = s + db * db;
+        float root = sqrtf(s);
+        sum = k == 0 ? root : sum + root;
+    }
+    float D = sum * (1.0f / 6.0f);
+    return D > a->corner_threshold;
+}
+
+/* tile_mask[Ty*Tx] (21 bits), cell_level[ceil(H/8)*ceil(W/8)], hist[4] (zeroed here).
+ * Mask bits: 0 = root split; 1+c = level-1 child c split (c = cx + 2cy); 5+4c+g = level-2
+ * grandchild g of child c split (g = gx + 2gy).  Top-down: a node is evaluated only if its
+ * parent split.  Level-3 nodes (8x8) never split.                                      */
+int32_t oracle_quadtree(const float *image, int32_t width, int32_t height, int32_t metric,
+                        uint32_t var_threshold_q, float corner_threshold, uint32_t *tile_mask,
+                        uint8_t *cell_level, uint32_t *hist)
+{
+    qt_args a = {image, width, height, metric, var_threshold_q, corner_threshold};
+    int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
+    int cells_x = (width + 7) / 8, cells_y = (height + 7) / 8;
+    uint64_t h[4] = {0, 0, 0, 0};
+    for (int ty = 0; ty < Ty; ++ty)
+        for (int tx = 0; tx < Tx; ++tx) {
+            int X = tx * 64, Y = ty * 64;
+            uint32_t mask = 0;
+            uint8_t lvl[8][8];                       /* leaf level of each 8x8 cell of the tile */
+            memset(lvl, 0, sizeof lvl);
+            if (node_splits(&a, X, Y, 64)) {
+                mask |= 1u;
+                for (int c = 0; c < 4; ++c) {
+                    int cx = X + 32 * (c & 1), cy = Y + 32 * (c >> 1);
+                    int child_split = node_splits(&a, cx, cy, 32);
+                    if (child_split) mask |= 1u << (1 + c);
+                    for (int g = 0; g < 4; ++g) {
+                        int gx = cx + 16 * (g & 1), gy = cy + 16 * (g >> 1);
+                        int level = 1;
+                        if (child_split) {
+                            level = 2;
+                            if (node_splits(&a, gx, gy, 16)) {
+                                mask |= 1u << (5 + 4 * c + g);
+                                level = 3;
+                            }
+                        }
+                        for (int v = 0; v < 2; ++v)
+                            for (int u = 0; u < 2; ++u)
+                                lvl[(gy - Y) / 8 + v][(gx - X) / 8 + u] = (uint8_t)level;
+                    }
+                }
+            }
+            if (tile_mask) tile_mask[ty * Tx + tx] = mask;
+            /* histogram: leaves that contain >= 1 in-image pixel, counted once each           */
+            for (int level = 0; level < 4; ++level) {
+                int side = 64 >> level, per = 1 << level;
+                for (int ny = 0; ny < per; ++ny)
+                    for (int nx = 0; nx < per; ++nx) {
+                        int x0 = X + nx * side, y0 = Y + ny * side;
+                        if (x0 >= width || y0 >= height) continue;
+                        if (lvl[(y0 - Y) / 8][(x0 - X) / 8] != level) continue;
+                        /* a leaf at `level` is the node whose own level equals the cell's    */
+                        h[level] += 1;
+                    }
+            }
+            for (int v = 0; v < 8; ++v)
+                for (int u = 0; u < 8; ++u) {
+                    int cxg = X / 8 + u, cyg = Y / 8 + v;
+                    if (cxg < cells_x && cyg < cells_y && cell_level)
+                        cell_level[cyg * cells_x + cxg] = lvl[v][u];
+                }
+        }
+    if (hist) for (int k = 0; k < 4; ++k) hist[k] = (uint32_t)h[k];
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O8 reprojection ("reprojecting pixels using the nearest available depth and the       */
+/* previous view-projection matrix"; P:53 first-fragment depth reused).  All fp32, operations  */
+/* exactly in this order; every fmaf is a real fused op; nothing else is contracted.           */
+/* ---------------------------------------------------------------------------------------- */
+int32_t oracle_reproject(int32_t width, int32_t height, const float *M, float depth_threshold,
+                         const float *background, const float *prev_trans,
+                         const float *prev_depth, const float *cur_depth, float *out_trans,
+                         float *out_depth, float *out_final, uint8_t *accept,
+                         uint32_t *reject_list, uint32_t *reject_count)
+{
+    uint32_t nrej = 0;
+    float fW = (float)width, fH = (float)height;
+    float inv_w = 1.0f / fW, inv_h = 1.0f / fH;
+    for (int y = 0; y < height; ++y)
+        for (int x = 0; x < width; ++x) {
+            size_t p = (size_t)y * width + x;
+            float xn = fmaf(2.0f * ((float)x + 0.5f), inv_w, -1.0f);
+            float yn = fmaf(2.0f * ((float)y + 0.5f), inv_h, -1.0f);
+            float d = cur_depth[p];
+            float c[4];
+            for (int k = 0; k < 4; ++k)
+                c[k] = fmaf(M[4 * k + 0], xn,
+                            fmaf(M[4 * k + 1], yn, fmaf(M[4 * k + 2], d, M[4 * k + 3])));
+            int ok = c[3] > 0.0f;
+            float d_e = 0.0f;
+            size_t q = 0;
+            if (ok) {
+                float xp = c[0] / c[3], yp = c[1] / c[3];
+                d_e = c[2] / c[3];
+                float fx = floorf((xp + 1.0f) * 0.5f * fW);
+                float fy = floorf((yp + 1.0f) * 0.5f * fH);
+                ok = (fx >= 0.0f) && (fx < fW) && (fy >= 0.0f) && (fy < fH);
+                if (ok) {
+                    q = (size_t)(int)fy * width + (size_t)(int)fx;
+                    ok = fabsf(prev_depth[q] - d_e) <= depth_threshold;
+                }
+            }
+            if (ok) {
+                for (int k = 0; k < 4; ++k) out_trans[4 * p + k] = prev_trans[4 * q + k];
+                if (out_depth) out_depth[p] = d_e;
+                if (out_final) {
+                    float t = prev_trans[4 * q + 3];
+                    for (int k = 0; k < 3; ++k)
+                        out_final[4 * p + k] =
+                            (float)((double)prev_trans[4 * q + k] + (double)t * (double)background[k]);
+                    out_final[4 * p + 3] = (float)(1.0 - (double)t);
+                }
+                if (accept) accept[p] = 1;
+            } else {
+                if (accept) accept[p] = 0;
+                if (reject_list) reject_list[nrej] = (uint32_t)p;
+                ++nrej;
+            }
+        }
+    if (reject_count) *reject_count = nrej;
+    return 0;
+}
+
+int32_t oracle_num_threads(void)
+{
+    int n = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp single
+        n = omp_get_num_threads();
+    }
+#endif
+    return n;
+}

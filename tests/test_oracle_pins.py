@@ -1,0 +1,616 @@
+"""Pins for the CPU oracle (SURVEY.md §8(c) "Pins"): what fixes each part of oracle/ against
+something other than itself -- brute force, closed forms, invariants, library routines.
+
+Runs on CPU (`-m "not gpu"`).  Nothing here touches the CUDA path.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import noit_scenes
+import oracle
+from noit_scenes.raster import FragBuf
+
+BG = (0.2, 0.3, 0.4)
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_facts.json")
+
+
+def close(a, b, rel=1e-5, abs_=1e-6):
+    """SURVEY §8(c) A24 tolerance: |a-b| <= 1e-5*max(|a|,|b|) + 1e-6."""
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    return np.all(np.abs(a - b) <= rel * np.maximum(np.abs(a), np.abs(b)) + abs_)
+
+
+def make_fb(counts, depth, rgba, width=None, height=1):
+    counts = np.asarray(counts, np.int64)
+    width = counts.size // height if width is None else width
+    off = np.zeros(counts.size + 1, np.uint32)
+    off[1:] = np.cumsum(counts)
+    return FragBuf(width, height, off, np.ascontiguousarray(depth, np.float32),
+                   np.ascontiguousarray(rgba))
+
+
+def random_tiny_pixels(rng, n_pix, max_n, tie_set=None, dtype=np.float32):
+    counts = rng.integers(0, max_n + 1, n_pix)
+    F = int(counts.sum())
+    if tie_set is None:
+        depth = rng.uniform(0.01, 0.99, F).astype(np.float32)
+    else:
+        depth = rng.choice(np.asarray(tie_set, np.float32), F)
+    rgba = rng.uniform(0.0, 1.0, (F, 4)).astype(dtype)
+    return make_fb(counts, depth, rgba)
+
+
+# -------------------------------------------------------------------------------------------
+# paper-fixed facts
+# -------------------------------------------------------------------------------------------
+def test_paper_facts():
+    g = json.load(open(GOLD))
+    sizes = g["mlp_layers"]["value"]
+    n_params = sum(a * b + b for a, b in zip(sizes[:-1], sizes[1:]))
+    assert n_params == noit_scenes.MLP_PARAMS == 771
+    assert noit_scenes.mlp_weights(0).shape == (771,)
+    # 10-feature DFAOIT net of the same shape would have 931 parameters (context)
+    assert 10 * 32 + 32 + 32 * 16 + 16 + 16 * 3 + 3 == 931
+    assert g["quadtree_mask_bits"]["value"] == 1 + 4 + 16
+    for row in ("Smoke", "Hairball"):                          # Table 1 row sums
+        r = g["table1_rows_ms"][row]
+        assert abs(r["pass1"] + r["pass2"] + r["pass3"] + r["inf_dfaoit"] - r["total_dfaoit"]) < 2e-3
+
+
+# -------------------------------------------------------------------------------------------
+# O1 selection / O2 counts: brute force with a stable sort
+# -------------------------------------------------------------------------------------------
+def brute_top2(fb):
+    off = fb.offsets.astype(np.int64)
+    i1 = np.full(fb.num_pixels, oracle.ABSENT, np.uint32)
+    i2 = np.full(fb.num_pixels, oracle.ABSENT, np.uint32)
+    for p in range(fb.num_pixels):
+        d = fb.depth[off[p]:off[p + 1]]
+        order = np.argsort(d, kind="stable")       # stable => index tie-break
+        if d.size >= 1:
+            i1[p] = order[0]
+        if d.size >= 2:
+            i2[p] = order[1]
+    return i1, i2
+
+
+def test_selection_bruteforce_cfg1(cfg1_scene):
+    fb = cfg1_scene.full
+    o = oracle.build_features(fb)
+    i1, i2 = brute_top2(fb)
+    assert np.array_equal(o["idx1"], i1) and np.array_equal(o["idx2"], i2)
+    assert np.array_equal(o["count"], fb.counts())
+
+
+def test_selection_bruteforce_ties():
+    rng = np.random.default_rng(1)
+    fb = random_tiny_pixels(rng, 10000, 8, tie_set=[0.25, 0.5, 0.5000001, 0.75])
+    o = oracle.build_features(fb)
+    i1, i2 = brute_top2(fb)
+    assert np.array_equal(o["idx1"], i1) and np.array_equal(o["idx2"], i2)
+    assert np.array_equal(o["count"], fb.counts())
+    # the case the tie rule exists for: equal depths => lower index wins
+    fb2 = make_fb([3], [0.5, 0.5, 0.5], np.ones((3, 4), np.float32) * 0.5)
+    o2 = oracle.build_features(fb2)
+    assert (o2["idx1"][0], o2["idx2"][0]) == (0, 1)
+    fb3 = make_fb([3], [0.7, 0.5, 0.5], np.ones((3, 4), np.float32) * 0.5)
+    o3 = oracle.build_features(fb3)
+    assert (o3["idx1"][0], o3["idx2"][0]) == (1, 2)
+
+
+def test_empty_and_single_pixels():
+    rgba = np.array([[0.9, 0.1, 0.2, 0.6]], np.float32)
+    fb = make_fb([0, 1, 0], [0.3], rgba)
+    o = oracle.build_features(fb)
+    assert list(o["idx1"]) == [oracle.ABSENT, 0, oracle.ABSENT]
+    assert list(o["idx2"]) == [oracle.ABSENT] * 3
+    assert list(o["depth1"]) == [1.0, np.float32(0.3), 1.0]
+    assert np.array_equal(o["features"][0], [0, 1, 0, 0, 0])
+    assert np.array_equal(o["features"][1], [1, 1, 0, 0, 0])
+    w = oracle.effective_weights(noit_scenes.mlp_weights(3), 0)
+    r = oracle.resolve(fb, w, BG)
+    # A10: empty pixel -> C_t = 0, T_tot = 1, C_p = background, coverage 0
+    assert np.array_equal(r["trans"][0], [0, 0, 0, 1])
+    assert close(r["final"][0], [*BG, 0.0])
+    assert close(r["trans"][1], [0.6 * 0.9, 0.6 * 0.1, 0.6 * 0.2, 0.4])
+
+
+# -------------------------------------------------------------------------------------------
+# O2 sums: identities and closed forms
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [np.float32, np.float16])
+def test_tail_identities(dtype):
+    rng = np.random.default_rng(2)
+    fb = random_tiny_pixels(rng, 3000, 40, dtype=dtype)
+    o = oracle.build_features(fb)
+    off = fb.offsets.astype(np.int64)
+    rg = fb.rgba.astype(np.float64)
+    for p in range(fb.num_pixels):
+        c = rg[off[p]:off[p + 1]]
+        tot_c = (c[:, 3:4] * c[:, :3]).sum(0)
+        tot_t = np.prod(1.0 - c[:, 3])
+        l1, l2 = o["layer1"][p].astype(np.float64), o["layer2"][p].astype(np.float64)
+        cacc, atail, ttail = o["tail_raw"][p, :3], o["tail_raw"][p, 3], o["tail_raw"][p, 4]
+        assert close(l1[3] * l1[:3] + l2[3] * l2[:3] + cacc, tot_c, 2e-6, 1e-6)
+        assert close((1 - l1[3]) * (1 - l2[3]) * ttail, tot_t, 2e-6, 1e-7)
+        assert close(l1[3] + l2[3] + atail, c[:, 3].sum(), 2e-6, 1e-6)
+        n = c.shape[0]
+        if n >= 1:  # layer 1 really is the fragment the brute force picks
+            j = np.argsort(fb.depth[off[p]:off[p + 1]], kind="stable")[0]
+            assert np.array_equal(o["layer1"][p], fb.rgba[off[p] + j].astype(np.float32))
+
+
+def test_tail_closed_forms():
+    # all tail colours = c  =>  C~_pm = c ;  all alpha = a  =>  T_tail = (1-a)^(N-2), A_tail = (N-2)a
+    for n in (3, 4, 17, 128):
+        a = 0.25
+        col = np.array([0.125, 0.5, 0.75])
+        rgba = np.zeros((n, 4), np.float32)
+        rgba[:, :3] = col
+        rgba[:, 3] = a
+        depth = np.linspace(0.9, 0.1, n).astype(np.float32)   # reverse order: nearest is LAST
+        fb = make_fb([n], depth, rgba)
+        o = oracle.build_features(fb)
+        assert (o["idx1"][0], o["idx2"][0]) == (n - 1, n - 2)
+        assert close(o["tail_raw"][0, 3], (n - 2) * a)
+        assert close(o["tail_raw"][0, 4], (1 - a) ** (n - 2), 1e-6, 1e-12)
+        assert close(o["features"][0], [n, (1 - a) ** (n - 2), *col])
+
+
+# -------------------------------------------------------------------------------------------
+# O4 MLP against a textbook float64 numpy forward pass; bf16 rounding against torch
+# -------------------------------------------------------------------------------------------
+def numpy_mlp(w, x):
+    w = w.astype(np.float64)
+    W1, b1 = w[:160].reshape(32, 5), w[160:192]
+    W2, b2 = w[192:704].reshape(16, 32), w[704:720]
+    W3, b3 = w[720:768].reshape(3, 16), w[768:771]
+    h = np.maximum(x.astype(np.float64) @ W1.T + b1, 0)
+    h = np.maximum(h @ W2.T + b2, 0)
+    return np.maximum(h @ W3.T + b3, 0)
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_mlp_vs_numpy(precision):
+    rng = np.random.default_rng(4)
+    w = noit_scenes.mlp_weights(7)
+    weff = oracle.effective_weights(w, precision)
+    x = np.concatenate([rng.integers(0, 137, (4000, 1)).astype(np.float32),
+                        rng.uniform(0, 1, (4000, 4)).astype(np.float32)], axis=1)
+    got = oracle.infer(weff, x)
+    assert close(got, numpy_mlp(weff, x), 1e-6, 1e-7)
+    assert (got > 0).mean() > 0.3           # the output ReLU is alive (b3 += 0.25)
+    # a transposed weight matrix or a swapped layer must fail this pin:
+    wrong = weff.copy()
+    wrong[:160] = weff[:160].reshape(32, 5).T.ravel()
+    assert not close(oracle.infer(wrong, x), got, 1e-3, 1e-3)
+
+
+def test_mlp_zero_weights_gives_relu_bias():
+    w = np.zeros(771, np.float32)
+    w[768:771] = [0.5, -0.25, 0.125]
+    x = np.random.default_rng(0).uniform(0, 100, (16, 5)).astype(np.float32)
+    out = oracle.infer(w, x)
+    assert np.array_equal(out, np.tile(np.float32([0.5, 0.0, 0.125]), (16, 1)))
+
+
+def test_bf16_rounding_matches_torch():
+    import torch
+    rng = np.random.default_rng(5)
+    w = np.concatenate([noit_scenes.mlp_weights(1), rng.normal(size=4000).astype(np.float32),
+                        np.float32([0.0, -0.0, 1.0, 1.00390625, 1.01171875, 3.0e-39])])
+    pad = np.zeros(771 * ((w.size + 770) // 771), np.float32)
+    pad[:w.size] = w
+    got = np.concatenate([oracle.effective_weights(pad[i:i + 771], 1)
+                          for i in range(0, pad.size, 771)])
+    ref = torch.from_numpy(pad).to(torch.bfloat16).to(torch.float32).numpy()
+    assert np.array_equal(got.view(np.uint32), ref.view(np.uint32))
+
+
+# -------------------------------------------------------------------------------------------
+# O5 composite (Eq. 4) and O5x exact reference (Eq. 1)
+# -------------------------------------------------------------------------------------------
+def python_over(depth, rgba, bg):
+    """Second brute force: insertion sort + recursive over operator C <- C + T*a*C_i; T <- T(1-a)."""
+    items = []
+    for j in range(len(depth)):
+        k = len(items)
+        while k > 0 and items[k - 1][0] > depth[j]:     # strict '>' keeps equal depths in index order
+            k -= 1
+        items.insert(k, (float(depth[j]), [float(v) for v in rgba[j]]))
+    C, T = [0.0, 0.0, 0.0], 1.0
+    for _, c in items:
+        for ch in range(3):
+            C[ch] += T * c[3] * c[ch]
+        T *= 1.0 - c[3]
+    return [C[ch] + T * bg[ch] for ch in range(3)] + [1.0 - T]
+
+
+def test_exact_reference_vs_python_bruteforce():
+    rng = np.random.default_rng(6)
+    fb = random_tiny_pixels(rng, 400, 9, tie_set=[0.1, 0.2, 0.3, 0.4, 0.5])
+    ex = oracle.exact(fb, BG)
+    off = fb.offsets.astype(np.int64)
+    for p in range(fb.num_pixels):
+        ref = python_over(fb.depth[off[p]:off[p + 1]], fb.rgba[off[p]:off[p + 1]], BG)
+        assert close(ex["final"][p], ref, 1e-6, 1e-7)
+
+
+def test_empty_tail_equals_exact_two_layer_composite():
+    """BASELINE.json invariant: with zero tail fragments the output equals exact front-to-back
+    compositing of the two peeled layers (reading A2 forces the tail term to 0)."""
+    rng = np.random.default_rng(7)
+    fb = random_tiny_pixels(rng, 5000, 2)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(2), 0)
+    r = oracle.resolve(fb, w, BG)
+    ex = oracle.exact(fb, BG)
+    assert close(r["final"], ex["final"], 1e-6, 1e-7)
+    # and an all-alpha-0 tail contributes nothing either (A2: has_tail = A_tail > 0)
+    rgba = rng.uniform(0, 1, (5, 4)).astype(np.float32)
+    rgba[2:, 3] = 0.0
+    fb2 = make_fb([5], [0.1, 0.2, 0.3, 0.4, 0.5], rgba)
+    assert close(oracle.resolve(fb2, w, BG)["final"], oracle.exact(fb2, BG)["final"], 1e-6, 1e-7)
+
+
+def test_exact_tail_identity_pins_eq4_structure():
+    """Replace f(x) by the exact tail composite: Eq. 4 must then equal Eq. 1 on the whole list.
+    Pins the T_2 factor, C_exact,2 and the background term independently of any weights."""
+    rng = np.random.default_rng(8)
+    fb = random_tiny_pixels(rng, 3000, 24)
+    ex = oracle.exact(fb, BG)
+    r = oracle.resolve(fb, None, BG, tail_override=ex["tail"])
+    assert close(r["final"], ex["final"], 2e-6, 1e-6)
+    # total transmittance in out_trans.w and coverage in out_final.w
+    assert close(1.0 - r["trans"][:, 3], ex["final"][:, 3], 2e-6, 1e-6)
+    # a wrong factor (e.g. dropping T_2) must be caught by this pin
+    r_bad = oracle.resolve(fb, None, BG, tail_override=ex["tail"] * 1.5)
+    assert not close(r_bad["final"], ex["final"], 1e-3, 1e-3)
+
+
+def test_resolve_matches_numpy_restatement_on_cfg1(cfg1_scene):
+    """Whole-pixel check on cfg1: features -> numpy float64 MLP -> Eq. 4, from the oracle's own
+    layer outputs (pins the glue between O3, O4 and O5)."""
+    fb = cfg1_scene.full
+    w = oracle.effective_weights(cfg1_scene.weights, 0)
+    o = oracle.build_features(fb)
+    f = numpy_mlp(w, o["features"])
+    l1, l2 = o["layer1"].astype(np.float64), o["layer2"].astype(np.float64)
+    a1, a2 = l1[:, 3:4], l2[:, 3:4]
+    t2 = (1 - a1) * (1 - a2)
+    has_tail = (o["tail_raw"][:, 3:4] > 0)
+    ct = a1 * l1[:, :3] + (1 - a1) * a2 * l2[:, :3] + np.where(has_tail, t2 * f, 0.0)
+    ttot = t2[:, 0] * o["tail_raw"][:, 4]
+    r = oracle.resolve(fb, w, BG)
+    assert close(r["trans"][:, :3], ct, 2e-6, 1e-6) and close(r["trans"][:, 3], ttot, 2e-6, 1e-7)
+    assert close(r["final"][:, :3], ct + ttot[:, None] * np.array(BG), 2e-6, 1e-6)
+    assert np.array_equal(r["depth1"], o["depth1"])
+    assert has_tail.mean() > 0.3
+
+
+# -------------------------------------------------------------------------------------------
+# O6 quadtree
+# -------------------------------------------------------------------------------------------
+def popcount(x):
+    return bin(int(x)).count("1")
+
+
+def check_mask_invariants(q, W, H):
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    for t, m in enumerate(q["tile_mask"]):
+        m = int(m)
+        assert m < (1 << 21)
+        for c in range(4):
+            if (m >> (1 + c)) & 1:
+                assert m & 1                                   # child bit => parent bit
+            for g in range(4):
+                if (m >> (5 + 4 * c + g)) & 1:
+                    assert (m >> (1 + c)) & 1
+    if W % 64 == 0 and H % 64 == 0:
+        # leaves = 1 + 3 * popcount(mask) per tile; leaf areas tile the image
+        assert int(q["hist"].sum()) == sum(1 + 3 * popcount(m) for m in q["tile_mask"])
+        area = sum(int(q["hist"][l]) * (64 >> l) ** 2 for l in range(4))
+        assert area == W * H
+    lv = q["cell_level"].reshape((H + 7) // 8, (W + 7) // 8)
+    assert lv.max() <= 3
+
+
+def test_quadtree_constant_image_only_max_tiles():
+    """BASELINE.json invariant: a constant-colour image yields only maximum-size tiles."""
+    for (W, H) in ((64, 64), (200, 120), (1920 // 4, 1080 // 4)):
+        img = np.zeros((H * W, 4), np.float32)
+        img[:] = (0.3, 0.6, 0.9, 0.5)
+        for metric in (0, 1):
+            q = oracle.quadtree(img, W, H, metric, 0, 0.0)
+            Tx, Ty = (W + 63) // 64, (H + 63) // 64
+            assert not q["tile_mask"].any()
+            assert list(q["hist"]) == [Tx * Ty, 0, 0, 0]
+            assert not q["cell_level"].any()
+
+
+def test_quadtree_checkerboard_splits_everything():
+    W, H = 192, 128
+    yy, xx = np.mgrid[0:H, 0:W]
+    img = np.zeros((H, W, 4), np.float32)
+    img[..., :3] = ((xx + yy) & 1)[..., None]
+    q = oracle.quadtree(img.reshape(-1, 4), W, H, 0, 6, 0.0)
+    assert (q["tile_mask"] == 0x1FFFFF).all()
+    assert list(q["hist"]) == [0, 0, 0, 6 * 64]
+    assert (q["cell_level"] == 3).all()
+    check_mask_invariants(q, W, H)
+
+
+def test_quadtree_single_pixel_path_and_closed_form_variance():
+    """One differing pixel: exactly the root -> child -> grandchild path containing it splits
+    (3 bits) when the threshold is below the node variance 3*(n-1)/n^2 * 255^2 (n = node pixels)."""
+    W = H = 64
+    img = np.zeros((H, W, 4), np.float32)
+    px, py = 40, 21                     # child c = 1 (right, upper), grandchild g = gx+2gy
+    img[py, px, :3] = 1.0
+    c = (px // 32) + 2 * (py // 32)
+    g = ((px % 32) // 16) + 2 * ((py % 32) // 16)
+    var16 = 3 * (256 - 1) / 256 ** 2 * 255 ** 2       # smallest node on the path (16x16)
+    q = oracle.quadtree(img.reshape(-1, 4), W, H, 0, 0, 0.0)
+    assert int(q["tile_mask"][0]) == (1 | (1 << (1 + c)) | (1 << (5 + 4 * c + g)))
+    lv = q["cell_level"].reshape(8, 8)
+    assert lv[py // 8, px // 8] == 3 and lv[0, 0] == 1 and lv[7, 7] == 1
+    assert list(q["hist"]) == [0, 3, 3, 4]
+    check_mask_invariants(q, W, H)
+    # closed-form thresholds: 64x64 root variance = 3*(4095)/4096^2*255^2 = 47.6.. -> thr 47 splits,
+    # thr 48 does not; 32x32: 190.3; 16x16: 759.0
+    var64 = 3 * 4095 / 4096 ** 2 * 255 ** 2
+    var32 = 3 * 1023 / 1024 ** 2 * 255 ** 2
+    assert oracle.quadtree(img.reshape(-1, 4), W, H, 0, int(var64), 0.0)["tile_mask"][0] != 0
+    assert oracle.quadtree(img.reshape(-1, 4), W, H, 0, int(var64) + 1, 0.0)["tile_mask"][0] == 0
+    m = int(oracle.quadtree(img.reshape(-1, 4), W, H, 0, int(var64), 0.0)["tile_mask"][0])
+    assert m == (1 | (1 << (1 + c)) | (1 << (5 + 4 * c + g)))      # deeper nodes have larger variance
+    assert int(var32) > int(var64) and int(var16) > int(var32)
+
+
+def bigint_variance_splits(img, W, H, x0, y0, side, thr):
+    x1, y1 = min(x0 + side, W), min(y0 + side, H)
+    if x0 >= x1 or y0 >= y1:
+        return False
+    n, s1, s2 = 0, [0, 0, 0], [0, 0, 0]
+    for y in range(y0, y1):
+        for x in range(x0, x1):
+            for ch in range(3):
+                v = float(np.float32(255.0) * np.float32(min(max(img[y, x, ch], 0.0), 1.0)))
+                q = int(np.rint(np.float32(v)))           # round-half-even on the fp32 product
+                s1[ch] += q
+                s2[ch] += q * q
+            n += 1
+    return sum(n * s2[ch] - s1[ch] ** 2 for ch in range(3)) > thr * n * n
+
+
+def test_quadtree_bigint_bruteforce_on_cfg1(cfg1_scene):
+    fb = cfg1_scene.full
+    w = oracle.effective_weights(cfg1_scene.weights, 0)
+    img = oracle.resolve(fb, w, BG)["trans"]
+    W = H = 64
+    im = img.reshape(H, W, 4)
+    for thr in (6, 60, 600):
+        q = oracle.quadtree(img, W, H, 0, thr, 0.0)
+        m = 0
+        if bigint_variance_splits(im, W, H, 0, 0, 64, thr):
+            m |= 1
+            for c in range(4):
+                cx, cy = 32 * (c & 1), 32 * (c >> 1)
+                if bigint_variance_splits(im, W, H, cx, cy, 32, thr):
+                    m |= 1 << (1 + c)
+                    for g in range(4):
+                        if bigint_variance_splits(im, W, H, cx + 16 * (g & 1), cy + 16 * (g >> 1),
+                                                  16, thr):
+                            m |= 1 << (5 + 4 * c + g)
+        assert int(q["tile_mask"][0]) == m
+        check_mask_invariants(q, W, H)
+    assert int(oracle.quadtree(img, W, H, 0, 6, 0.0)["tile_mask"][0]) != 0
+
+
+def test_quadtree_partial_tiles_and_corner_metric():
+    W, H = 100, 72          # partial tiles: 100 = 64 + 36, 72 = 64 + 8
+    rng = np.random.default_rng(9)
+    img = rng.uniform(0, 1, (H, W, 4)).astype(np.float32)
+    q = oracle.quadtree(img.reshape(-1, 4), W, H, 0, 6, 0.0)
+    check_mask_invariants(q, W, H)
+    # leaves counted = leaves with >= 1 in-image pixel: noise splits everything in-image
+    assert q["hist"][3] == ((W + 7) // 8) * ((H + 7) // 8)
+    # corner metric: numpy restatement of the 6-pair mean distance on the root node of tile 0
+    im = img.astype(np.float64)
+    cs = [im[0, 0, :3], im[0, 63, :3], im[63, 0, :3], im[63, 63, :3]]
+    D = np.mean([np.linalg.norm(cs[a] - cs[b]) for a in range(4) for b in range(a + 1, 4)])
+    lo = oracle.quadtree(img.reshape(-1, 4), W, H, 1, 0, float(D) * 0.999)["tile_mask"][0] & 1
+    hi = oracle.quadtree(img.reshape(-1, 4), W, H, 1, 0, float(D) * 1.001)["tile_mask"][0] & 1
+    assert lo == 1 and hi == 0
+
+
+# -------------------------------------------------------------------------------------------
+# O7 adaptive resolve
+# -------------------------------------------------------------------------------------------
+def small_adaptive_scene(seed=0, W=128, H=128):
+    sc = noit_scenes.cfg3(seed, W=W, H=H, n_prims=40, mean_band=(9.0, 11.0), cap=32, coarse=True)
+    return sc
+
+
+def test_adaptive_all_fine_levels_is_plain_resolve():
+    sc = small_adaptive_scene()
+    w = oracle.effective_weights(sc.weights, 1)
+    plain = oracle.resolve(sc.full, w, BG)
+    cells = ((sc.full.width + 7) // 8) * ((sc.full.height + 7) // 8)
+    for lvl in (2, 3):
+        r = oracle.resolve(sc.full, w, BG, half=sc.half, quarter=sc.quarter,
+                           cell_level=np.full(cells, lvl, np.uint8))
+        for k in ("trans", "final", "depth1"):
+            assert np.array_equal(r[k], plain[k])
+
+
+def synthetic_coarse(W, H, r, field):
+    """Coarse buffer with exactly 3 fragments per coarse pixel (front, second, one tail fragment)
+    whose second-layer and tail colours follow `field(X, Y) -> (c2[3], ct[3])` in coarse coords."""
+    Wr, Hr = -(-W // r), -(-H // r)
+    depth, rgba = [], []
+    for Y in range(Hr):
+        for X in range(Wr):
+            c2, ct = field(X, Y)
+            depth += [0.1, 0.2, 0.3]
+            rgba += [[0.0, 0.0, 0.0, 0.5], [*c2, 0.5], [*ct, 0.25]]
+    fb = make_fb([3] * (Wr * Hr), depth, np.asarray(rgba, np.float32), width=Wr, height=Hr)
+    return fb
+
+
+def test_adaptive_bilinear_reproduces_affine_field_in_leaf_interior():
+    W = H = 64
+    # full-res buffer: one front fragment per pixel
+    front = np.array([0.8, 0.1, 0.3, 0.5], np.float32)
+    full = make_fb([1] * (W * H), np.full(W * H, 0.05, np.float32),
+                   np.tile(front, (W * H, 1)), width=W, height=H)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(11), 0)
+    for r, level in ((4, 0), (2, 1)):
+        def field(X, Y):
+            return ([0.1 + 0.01 * X, 0.2 + 0.005 * Y, 0.3], [0.2 + 0.02 * X, 0.9 - 0.01 * Y, 0.5])
+        cb = synthetic_coarse(W, H, r, field)
+        cells = np.full(64, level, np.uint8)
+        out = oracle.resolve(full, w, BG, half=cb if r == 2 else None,
+                             quarter=cb if r == 4 else None, cell_level=cells)
+        side = 64 >> level
+        tex = side // r
+        for (x, y) in ((10, 10), (17, 5), (side - 1 - r, r), (side // 2, side // 2 + 1)):
+            u, v = (x + 0.5) / r - 0.5, (y + 0.5) / r - 0.5
+            assert 0 <= u <= tex - 1 and 0 <= v <= tex - 1          # interior: no clamping
+            c2, ctail = field(u, v)                                    # affine => exact
+            a2C2 = 0.5 * np.array(c2)
+            x_feat = np.array([[3.0, 0.75, *ctail]], np.float32)       # N, T_tail=(1-.25), C_acc/A
+            f = numpy_mlp(w, x_feat)[0]
+            a1 = 0.5
+            ct = a1 * front[:3] + (1 - a1) * a2C2 + (1 - a1) * (1 - 0.5) * f
+            ttot = (1 - a1) * (1 - 0.5) * 0.75
+            p = y * W + x
+            assert close(out["trans"][p, :3], ct, 1e-5, 1e-6), (r, x, y)
+            assert close(out["trans"][p, 3], ttot)
+        # constant field: exact everywhere, including clamped borders
+        cbc = synthetic_coarse(W, H, r, lambda X, Y: ([0.3, 0.4, 0.5], [0.6, 0.7, 0.8]))
+        outc = oracle.resolve(full, w, BG, half=cbc if r == 2 else None,
+                              quarter=cbc if r == 4 else None, cell_level=cells)
+        assert np.ptp(outc["trans"], axis=0).max() < 1e-6
+
+
+def test_adaptive_taps_are_clamped_to_the_leaf():
+    """Tile independence (A19): coarse texels outside a pixel's own leaf never influence it."""
+    sc = small_adaptive_scene(3)
+    W, H = sc.full.width, sc.full.height
+    w = oracle.effective_weights(sc.weights, 1)
+    cells_x = (W + 7) // 8
+    cells = np.zeros(cells_x * ((H + 7) // 8), np.uint8)            # all 64-leaves -> quarter res
+    a = oracle.resolve(sc.full, w, BG, half=sc.half, quarter=sc.quarter, cell_level=cells)
+    # scramble the quarter-res colours of every coarse texel outside leaf (0,0) [texels 0..15]
+    q2 = FragBuf(sc.quarter.width, sc.quarter.height, sc.quarter.offsets, sc.quarter.depth,
+                 sc.quarter.rgba.copy())
+    off = q2.offsets.astype(np.int64)
+    for Y in range(q2.height):
+        for X in range(q2.width):
+            if X >= 16 or Y >= 16:
+                pq = Y * q2.width + X
+                q2.rgba[off[pq]:off[pq + 1]] = np.float16(0.5)
+    b = oracle.resolve(sc.full, w, BG, half=sc.half, quarter=q2, cell_level=cells)
+    A = a["trans"].reshape(H, W, 4)
+    B = b["trans"].reshape(H, W, 4)
+    assert np.array_equal(A[:64, :64], B[:64, :64])
+    assert not np.array_equal(A[:64, 64:], B[:64, 64:])
+    # and the result differs from the plain resolve (it really used the coarse data)
+    assert not np.array_equal(a["trans"], oracle.resolve(sc.full, w, BG)["trans"])
+    # layer 1 stays full-res: depth1 identical to the plain resolve
+    assert np.array_equal(a["depth1"], oracle.resolve(sc.full, w, BG)["depth1"])
+
+
+# -------------------------------------------------------------------------------------------
+# O8 reprojection / O9 fallback
+# -------------------------------------------------------------------------------------------
+def random_frame(rng, W, H):
+    trans = rng.uniform(0, 1, (W * H, 4)).astype(np.float32)
+    depth = rng.uniform(0.05, 0.95, W * H).astype(np.float32)
+    return trans, depth
+
+
+def test_reproject_identity_is_identity():
+    """BASELINE.json invariant: identity-camera reprojection is the identity (bitwise)."""
+    rng = np.random.default_rng(10)
+    for (W, H) in ((64, 64), (317, 203), (1920, 1080)):
+        trans, depth = random_frame(rng, W, H)
+        r = oracle.reproject(W, H, np.eye(4), 1e-3, BG, trans, depth, depth)
+        assert r["accept"].all() and r["reject_count"] == 0
+        assert np.array_equal(r["trans"], trans)
+        assert np.array_equal(r["depth"], depth)
+        assert close(r["final"][:, :3], trans[:, :3] + trans[:, 3:4] * np.array(BG), 1e-6, 1e-7)
+
+
+def test_reproject_integer_shift():
+    rng = np.random.default_rng(11)
+    W, H = 128, 64                      # power-of-two sizes: the NDC shift is exact in fp32
+    trans, depth = random_frame(rng, W, H)
+    for (kx, ky) in ((3, 0), (-5, 2), (0, -7)):
+        M = np.eye(4)
+        M[0, 3] = 2.0 * kx / W          # previous pixel = current pixel + (kx, ky)
+        M[1, 3] = 2.0 * ky / H
+        depth_flat = np.full(W * H, 0.5, np.float32)
+        r = oracle.reproject(W, H, M, 1e-3, BG, trans, depth_flat, depth_flat)
+        T = trans.reshape(H, W, 4)
+        out = r["trans"].reshape(H, W, 4)
+        acc = r["accept"].reshape(H, W)
+        yy, xx = np.mgrid[0:H, 0:W]
+        inside = (xx + kx >= 0) & (xx + kx < W) & (yy + ky >= 0) & (yy + ky < H)
+        assert np.array_equal(acc.astype(bool), inside)
+        ys, xs = np.nonzero(inside)
+        assert np.array_equal(out[ys, xs], T[ys + ky, xs + kx])
+        assert r["reject_count"] == int((~inside).sum())
+        assert set(r["reject_list"].tolist()) == set((yy[~inside] * W + xx[~inside]).tolist())
+        assert not out[~inside].any()                  # rejected pixels untouched
+
+
+def test_reproject_depth_threshold_and_w_sign():
+    W = H = 16
+    rng = np.random.default_rng(12)
+    trans, _ = random_frame(rng, W, H)
+    cur = np.full(W * H, 0.5, np.float32)
+    prev = cur.copy()
+    tau = 1e-3
+    prev[5] = np.float32(0.5) + np.float32(0.5 * tau)       # inside the threshold
+    prev[6] = np.float32(0.5) + np.float32(2.0 * tau)       # outside
+    prev[7] = np.float32(0.5) - np.float32(2.0 * tau)       # outside (other side)
+    r = oracle.reproject(W, H, np.eye(4), tau, BG, trans, prev, cur)
+    assert r["accept"][5] == 1 and r["accept"][6] == 0 and r["accept"][7] == 0
+    assert r["reject_count"] == 2
+    M = np.eye(4)
+    M[3, 3] = -1.0                                           # c_3 <= 0 everywhere
+    r2 = oracle.reproject(W, H, M, tau, BG, trans, prev, cur)
+    assert not r2["accept"].any() and r2["reject_count"] == W * H
+    M[3, 3] = 0.0
+    assert not oracle.reproject(W, H, M, tau, BG, trans, prev, cur)["accept"].any()
+
+
+def test_fallback_covers_every_pixel_once(cfg1_scene):
+    """O9: accepted U resolved = every pixel exactly once; tau_d < 0 => plain resolve bitwise."""
+    fb = cfg1_scene.full
+    W = H = 64
+    w = oracle.effective_weights(cfg1_scene.weights, 0)
+    plain = oracle.resolve(fb, w, BG)
+    M = np.eye(4)
+    M[0, 3] = 2.0 * 4 / W
+    rp = oracle.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"])
+    acc = rp["accept"].astype(bool)
+    assert 0 < rp["reject_count"] < W * H
+    assert np.array_equal(np.sort(rp["reject_list"]), np.nonzero(~acc)[0])
+    out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+    oracle.resolve(fb, w, BG, pixel_list=rp["reject_list"], out=out)
+    assert np.array_equal(out["trans"][~acc], plain["trans"][~acc])
+    assert np.array_equal(out["final"][~acc], plain["final"][~acc])
+    # everything rejected -> the frame equals a plain resolve bitwise
+    rp2 = oracle.reproject(W, H, np.eye(4), -1.0, BG, plain["trans"], plain["depth1"],
+                           plain["depth1"])
+    assert rp2["reject_count"] == W * H
+    out2 = dict(trans=rp2["trans"], final=rp2["final"], depth1=rp2["depth"])
+    oracle.resolve(fb, w, BG, pixel_list=rp2["reject_list"], out=out2)
+    for k in ("trans", "final", "depth1"):
+        assert np.array_equal(out2[k], plain[k])
