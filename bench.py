@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the neural-OIT hot path on B200 (contract: see DESIGN.md §Measurement).
+
+One STEP = one pass of the whole hot path over the 1080p high-depth-
+complexity workload (BASELINE.json configs[2], "cfg3", plus the half/quarter buffers of the same
+primitives):
+   1. noit_resolve   plain fused resolve of the frame (S1-S5)          <- dominant kernel
+   2. noit_quadtree  colour-variance tiles of its result (S6)
+   3. noit_resolve   adaptive resolve guided by those tiles (S7)
+   4. noit_reproject previous result under a small camera motion (S8)
+   5. noit_resolve   fallback resolve of the rejected pixels (S9)
+and produces three output frames, so `value` = 3*P pixels / step time.  The plain fused resolve
+alone (the metric BASELINE.json names: Mpixels/s and fragments/s at 1080p, % of HBM roofline) is
+timed with its own CUDA events inside the same timed region and reported in `roofline` and in
+`resolve_*`.  Inputs (647 MB) are larger than L2 (126 MB), so no flush is needed between steps.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+BG = (0.2, 0.3, 0.4)
+WORKLOAD = "cfg3: 1920x1080, 512 ellipses, mean 24 / max 128 fragments per pixel, RGBA fp16, bf16 weights"
+METRIC = "Mpixels/s of neural OIT resolve at 1080p (whole hot path S1-S9 per step)"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.samples, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def camera_shift_matrix(W: int, H: int) -> np.ndarray:
+    """Small camera motion for step 4: NDC translation of (1.5, 0.5) pixels, depth untouched."""
+    M = np.eye(4, dtype=np.float64)
+    M[0, 3] = 2.0 * 1.5 / W
+    M[1, 3] = 2.0 * 0.5 / H
+    return M.astype(np.float32)
+
+
+def resolve_bytes(P: int, F: int, color_bytes: int, n_images: int, depth1: bool) -> int:
+    """Algorithmic bytes of the fused resolve: offsets + fragments + outputs."""
+    return 4 * (P + 1) + F * (4 + color_bytes) + 16 * P * n_images + (4 * P if depth1 else 0)
+
+
+def dist_setup(n_gpus: int, backend: str):
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group(backend=backend)
+        return dist, dist.get_rank(), world
+    return None, 0, 1
+
+
+def max_over_ranks(dist, value: float, device) -> float:
+    import torch
+    if dist is None:
+        return value
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def run_dryrun(args):
+    """CPU/gloo exercise of the N>1 plumbing (tests/test_abi.py): no GPU work, no numbers."""
+    import torch
+    dist, rank, world = dist_setup(args.gpus, "gloo")
+    t = torch.ones(1)
+    if dist is not None:
+        dist.barrier()
+        dist.all_reduce(t)
+    ms = max_over_ranks(dist, 1.0 + rank, "cpu")
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": None, "n_gpus": world, "dryrun": True,
+                          "scaling": "weak", "ranks_seen": int(t.item()), "ms_per_step": ms}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def oracle_step(oracle, sc, w_eff, M, state):
+    """The same five calls as the GPU step, on the CPU oracle (reference arm / cpu_baseline)."""
+    fbh = sc.full
+    W, H = fbh.width, fbh.height
+    r = oracle.resolve(fbh, w_eff, BG)
+    qt = oracle.quadtree(r["final"], W, H, 0, 6)
+    oracle.resolve(fbh, w_eff, BG, half=sc.half, quarter=sc.quarter, cell_level=qt["cell_level"])
+    rp = oracle.reproject(W, H, M, 1e-3, BG, r["trans"], r["depth1"], r["depth1"])
+    out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+    oracle.resolve(fbh, w_eff, BG, pixel_list=rp["reject_list"], out=out)
+    state["rejected"] = rp["reject_count"]
+
+
+def run_reference(args):
+    """`--impl reference`: the oracle, as it stands, on the host cores; each step = the whole
+    path on a bounded sample (the top `rows` pixel rows of the same cfg3 frame)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import noit_scenes
+    import oracle
+    sc = noit_scenes.cfg3(0, coarse=True)
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    t0 = time.perf_counter()
+    oracle_step(oracle, sc, w_eff, camera_shift_matrix(sc.full.width, sc.full.height), {})
+    if time.perf_counter() - t0 > 4.0:           # slow host: bounded sample = a 256-row band
+        y0, y1 = 384, 640
+        sc = noit_scenes.Scene("cfg3-band", sc.full.rows(y0, y1), sc.half.rows(y0 // 2, y1 // 2),
+                               sc.quarter.rows(y0 // 4, y1 // 4), sc.weights, sc.mlp_precision)
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    M = camera_shift_matrix(sc.full.width, sc.full.height)
+    state = {}
+    for _ in range(args.warmup):
+        oracle_step(oracle, sc, w_eff, M, state)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(oracle, sc, w_eff, M, state)
+    dt = time.perf_counter() - t0
+    P = sc.full.num_pixels
+    value = 3 * P * args.steps / dt / 1e6
+    cores = oracle.num_threads()
+    sample = f"{sc.full.height} rows of the cfg3 frame ({P} pixels, {sc.full.num_fragments} fragments) per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "Mpixels/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "Mpixels/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "Mpixels/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+
+    import noit_scenes
+    import paper_2606_16747_b200 as noit
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist, rank, world = dist_setup(args.gpus, "nccl")
+
+    # weak scaling: every rank resolves its own 1080p frame (seed = rank), no data-path collective
+    sc = noit_scenes.cfg3(rank, coarse=True)
+    fbh = sc.full
+    W, H, P, F = fbh.width, fbh.height, fbh.num_pixels, fbh.num_fragments
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b, dev) for b in (sc.full, sc.half, sc.quarter))
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    M = camera_shift_matrix(W, H)
+    f32 = dict(dtype=torch.float32, device=dev)
+    plain = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
+    adapt = dict(final=torch.empty((P, 4), **f32))
+    qt = None
+    rp = None
+    d_plain = ctx.make_resolve_desc(fb, BG, plain["trans"], plain["final"], plain["depth1"])
+    stream = torch.cuda.current_stream()
+    names = ["resolve", "quadtree", "adaptive", "reproject", "fallback"]
+
+    def step(ev=None):
+        nonlocal qt, rp
+        if ev: ev[0].record(stream)
+        ctx.resolve_desc(d_plain)
+        if ev: ev[1].record(stream)
+        qt = ctx.quadtree(plain["final"], W, H, noit.QT_VARIANCE, 6, out=qt)
+        if ev: ev[2].record(stream)
+        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=qt["cell_level"])
+        if ev: ev[3].record(stream)
+        rp = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"], out=rp)
+        if ev: ev[4].record(stream)
+        ctx.resolve(fb, BG, want=(), out=dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"]),
+                    pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
+        if ev: ev[5].record(stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = ctx.launch_count
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(args.steps):
+        step(events[k])
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    launches = ctx.launch_count - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = events[0][0].elapsed_time(events[-1][5])
+    total_ms = max_over_ranks(dist, total_ms, dev)
+    per_kernel = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in events])) for i, n in enumerate(names)}
+    resolve_ms = max_over_ranks(dist, per_kernel["resolve"], dev)
+
+    # e2e: the same resolve through noit_resolve_host, pinned HOST buffers, copies inside the timing
+    h_off = torch.from_numpy(fbh.offsets.view(np.int32)).pin_memory()
+    h_depth = torch.from_numpy(fbh.depth).pin_memory()
+    h_rgba = torch.from_numpy(fbh.rgba).pin_memory()
+    h_final = torch.empty((P, 4), dtype=torch.float32).pin_memory()
+
+    class HostFB:
+        width, height, num_fragments, color_fmt = W, H, F, fb.color_fmt
+        offsets, depth, rgba = h_off, h_depth, h_rgba
+
+    e2e_steps = max(1, min(args.steps, 5))
+    ctx.resolve_host(HostFB, BG, out_final=h_final)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        ctx.resolve_host(HostFB, BG, out_final=h_final)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    e2e_ms = max_over_ranks(dist, e0.elapsed_time(e1) / e2e_steps, dev)
+    rejected = int(rp["reject_count"].item())
+    hist = qt["hist"].cpu().numpy().view(np.uint32).tolist()
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        ms_step = total_ms / args.steps
+        rbytes = resolve_bytes(P, F, 8, 2, True)
+        achieved = rbytes / (resolve_ms * 1e-3) / 1e9
+        rec = {
+            "metric": METRIC, "value": 3 * P * world / (ms_step * 1e-3) / 1e6, "unit": "Mpixels/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD, "pixels": P, "fragments": F, "frames_per_step": 3,
+                       "l2": "inputs (647 MB) larger than L2 (126 MB); no flush", "seed": "rank"},
+            "resolve_mpix_s": P * world / (resolve_ms * 1e-3) / 1e6,
+            "resolve_gfrag_s": F * world / (resolve_ms * 1e-3) / 1e9,
+            "kernel_ms": per_kernel,
+            "roofline": {"bound": "hbm", "kernel": "noit_resolve (plain fused, S1-S5)", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                         "algorithmic_bytes": rbytes, "traffic": None},
+            "e2e": {"value": P * world / (e2e_ms * 1e-3) / 1e6, "unit": "Mpixels/s",
+                    "what": "noit_resolve_host on the same frame, pinned host buffers",
+                    "h2d_bytes_per_step": 4 * (P + 1) + 12 * F, "d2h_bytes_per_step": 16 * P,
+                    "ms_per_step": e2e_ms},
+            "gpu_launches": launches, "clocks": clocks,
+            "tile_hist": hist, "rejected_fraction": rejected / P,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            rec["cpu_baseline"] = cpu_baseline(sc)
+        print(json.dumps(rec))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(sc) -> dict:
+    """The oracle as it stands on this box's host cores: plain resolve of the same frame,
+    repeated for about 10 s (bounded), same metric as `resolve_mpix_s`."""
+    import oracle
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    oracle.resolve(sc.full, w_eff, BG)
+    n, t0 = 0, time.perf_counter()
+    while n < 3 or (time.perf_counter() - t0 < 10.0 and n < 200):
+        oracle.resolve(sc.full, w_eff, BG)
+        n += 1
+    dt = (time.perf_counter() - t0) / n
+    return {"value": sc.full.num_pixels / dt / 1e6, "unit": "Mpixels/s", "cores": oracle.num_threads(),
+            "kind": "oracle", "ms_per_frame": dt * 1e3,
+            "sample": f"plain resolve (S1-S5) of the whole cfg3 frame, {n} repetitions"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if os.environ.get("NOIT_BENCH_DRYRUN"):
+        return run_dryrun(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

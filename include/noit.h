@@ -1,0 +1,182 @@
+/* noit.h -- C ABI of libnoit.so: B200-native (sm_100a) neural order-independent-transparency
+ * resolve, the hot path of STAR-NT (arxiv/paper_2606_16747).
+ *
+ * Citations: "P:n" = line n of PAPER.md; "S:8(x)" = SURVEY.md section 8(x); readings A1..A24
+ * and operation definitions O1..O9 are restated in DESIGN.md.
+ *
+ * Conventions
+ *  - Unless a function name ends in `_host`, every pointer INSIDE a descriptor is a DEVICE
+ *    pointer owned by the caller (e.g. a PyTorch tensor).  The library never frees or retains
+ *    caller memory.  Descriptors themselves, `M`, `background`, weights are HOST memory.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls enqueue
+ *    work on it and return without synchronising (except the `_host` entry points, which
+ *    return after their results are in the caller's host buffers).
+ *  - Every entry point returns noit_status.  Host-checkable errors (NULL pointers, bad sizes,
+ *    unknown enums, missing weights, misalignment) are detected BEFORE any launch and leave all
+ *    outputs untouched.  CUDA errors map to NOIT_ERR_CUDA with text in noit_last_error().
+ *  - Device-side preconditions are documented, not checked: offsets non-decreasing with
+ *    offsets[P] == num_fragments; depth finite; alpha in [0,1]; inputs and outputs do not alias
+ *    (except noit_reproject's cur_depth == prev_depth, which is allowed).
+ *  - A context is not thread-safe; distinct contexts are independent.
+ *  - There is no CPU fallback and no other backend.
+ *
+ * Fragment buffer layout (S:8(a) S0; stands in for the paper's three raster passes P:55):
+ *    offsets u32[P+1]   row-major pixels p = y*W + x, offsets[0] = 0, non-decreasing
+ *    depth   f32[F]     smaller = nearer (A9); 16-byte aligned base
+ *    rgba    half[F][4] or float[F][4], STRAIGHT colour, .w = alpha (A8); 16-byte aligned base
+ *  Fragments of a pixel are contiguous and in submission order; "fragment index" = position.
+ */
+#ifndef NOIT_H
+#define NOIT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct noit_ctx noit_ctx; /* opaque; owns the device copy of the weights + small scratch */
+
+typedef enum {
+    NOIT_OK = 0,
+    NOIT_ERR_NULL = 1,        /* a required pointer is NULL                                   */
+    NOIT_ERR_SIZE = 2,        /* width/height <= 0, P+1 or F overflow u32, count != 771, ...  */
+    NOIT_ERR_FORMAT = 3,      /* unknown enum value or misaligned pointer                     */
+    NOIT_ERR_NO_WEIGHTS = 4,  /* MLP needed but noit_set_weights was never called             */
+    NOIT_ERR_CUDA = 5,        /* a CUDA runtime call failed; see noit_last_error              */
+    NOIT_ERR_UNSUPPORTED = 6  /* valid request this build does not implement                  */
+} noit_status;
+
+enum { NOIT_RGBA_F16 = 0, NOIT_RGBA_F32 = 1 };     /* fragment colour format                  */
+enum { NOIT_MLP_FP32 = 0, NOIT_MLP_BF16 = 1 };     /* weight precision (A6)                   */
+enum { NOIT_QT_VARIANCE = 0, NOIT_QT_CORNER = 1 }; /* quadtree split metric (A14)             */
+
+#define NOIT_MLP_PARAMS 771        /* 5->32->16->3 with biases (A4)                     */
+#define NOIT_ABSENT 0xFFFFFFFFu    /* idx1/idx2 of a missing layer                            */
+
+typedef struct {
+    int32_t width, height;
+    uint32_t num_fragments;        /* F = offsets[P]                                          */
+    int32_t color_fmt;             /* NOIT_RGBA_F16 | NOIT_RGBA_F32                           */
+    const uint32_t* offsets;       /* [P+1]                                                   */
+    const float* depth;            /* [F]                                                     */
+    const void* rgba;              /* [F][4]                                                  */
+} noit_fragbuf;
+
+/* ---- context ------------------------------------------------------------------------------ */
+noit_status noit_create(noit_ctx** out);
+void noit_destroy(noit_ctx* ctx);
+/* host array of 771 floats: W1[32][5], b1[32], W2[16][32], b2[16], W3[3][16], b3[3] (row =
+ * output neuron).  precision NOIT_MLP_BF16 rounds every weight to bf16 (RNE) once, here,
+ * and widens it back; activations and accumulation stay fp32 (A6).  Synchronous.             */
+noit_status noit_set_weights(noit_ctx* ctx, const float* host_w, int32_t count, int32_t precision);
+/* copies the EFFECTIVE weights (after the rounding above) into host_out[771].                */
+noit_status noit_get_weights(const noit_ctx* ctx, float* host_out, int32_t count);
+/* static or ctx-owned string; never freed by the caller; ctx may be NULL.                    */
+const char* noit_last_error(const noit_ctx* ctx);
+/* number of kernels this context has launched so far (bench.py's gpu_launches).              */
+uint64_t noit_launch_count(const noit_ctx* ctx);
+
+/* ---- S1-S3: k=2 nearest-layer selection + tail reduction + features
+ * Any output pointer may be NULL (skipped); at least one must be set.
+ *   idx1, idx2  LOCAL index (j - offsets[p]) of the nearest / 2nd nearest fragment under the
+ *               key (depth, index), NOIT_ABSENT if the layer is missing (O1)
+ *   count       N = n_p
+ *   layer1/2    straight RGBA of the two layers, zeros if absent
+ *   depth1      depth of layer 1, 1.0f for an empty pixel (A10)
+ *   tail_raw    C_acc.rgb = sum a_i C_i, A_tail = sum a_i, T_tail = prod (1-a_i) over the tail
+ *               (every fragment that is not layer 1 or 2) (O2)
+ *   features    x = [N, T_tail, C_acc / A_tail] (zeros for the colour if A_tail == 0) (O3)  */
+typedef struct {
+    uint32_t* idx1; uint32_t* idx2; uint32_t* count;   /* [P] each                            */
+    float* layer1; float* layer2;                      /* [P][4]                              */
+    float* depth1;                                     /* [P]                                 */
+    float* tail_raw;                                   /* [P][5]                              */
+    float* features;                                   /* [P][5]                              */
+} noit_layers;
+noit_status noit_build_features(noit_ctx* ctx, const noit_fragbuf* fb, const noit_layers* out,
+                                void* stream);
+
+/* ---- S4 alone: f(x) = relu(W3 relu(W2 relu(W1 x + b1) + b2) + b3) on n rows (A3).
+ * No has_tail gating.  features [n][5] -> tail_rgb [n][3].  n == 0 is a no-op.               */
+noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* tail_rgb,
+                       void* stream);
+
+/* ---- S1-S5 fused resolve (Eq. 4; O5); S7 when cell_level is set (O7);
+ * S9 when pixel_list is set (O9).
+ *   C_t   = a1 C1 + (1-a1) a2 C2 + [A_tail > 0] T_2 f(x),  T_2 = (1-a1)(1-a2)
+ *   T_tot = T_2 T_tail;  C_p = C_t + T_tot C_b
+ *   out_trans  [P][4] = (C_t, T_tot)      out_final [P][4] = (C_p, 1 - T_tot)
+ *   out_depth1 [P]    = depth of layer 1, 1.0f if empty.   No clamping anywhere (A11).
+ * At least one output must be non-NULL; out_trans/out_final need 16-byte alignment.
+ * Adaptive (S7): cell_level[ceil(H/8)*ceil(W/8)] from noit_quadtree gives each 8x8 cell its
+ * leaf level; lod = level_to_lod[level] in {0,1,2}; lod 1 reads `half` (ceil(W/2) x
+ * ceil(H/2)), lod 2 reads `quarter`; layer 1 always comes from `full`; layer 2
+ * (premultiplied) and the raw tail accumulators of the coarse pixels are bilinearly upsampled
+ * with taps clamped to the pixel's own leaf, then features, MLP and composite run at full
+ * resolution (A18-A20).  A level that maps to lod k > 0 requires the matching buffer.
+ * pixel_list/pixel_count (device): resolve only the listed pixels (count read on the device),
+ * leave the others untouched; not combinable with cell_level.                                */
+typedef struct {
+    noit_fragbuf full;
+    const noit_fragbuf* half;        /* NULL => no S7                                          */
+    const noit_fragbuf* quarter;
+    const uint8_t* cell_level;       /* NULL => plain resolve                                  */
+    uint8_t level_to_lod[4];         /* default {2,1,0,0}: 64-leaf->1/4, 32->1/2, 16/8->full   */
+    float background[3];             /* C_b (A11)                                              */
+    const uint32_t* pixel_list;      /* [<= P] pixel indices, or NULL                          */
+    const uint32_t* pixel_count;     /* device scalar: entries of pixel_list to process        */
+    float* out_trans; float* out_final; float* out_depth1;
+} noit_resolve_desc;
+noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* desc, void* stream);
+
+/* Same as noit_resolve (plain, no S7/S9) but EVERY pointer in `desc` is a HOST pointer: the
+ * call stages the fragment buffer into context-owned device memory (grown on demand, kept
+ * between calls), runs the fused kernel and copies the requested outputs back.  Returns after
+ * the outputs are in host memory.  Pinned host memory makes the copies asynchronous DMA.     */
+noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* host_desc, void* stream);
+
+/* ---- S6 quadtree split (sizes 64->8 per BASELINE.json cfg4, A13; O6).
+ * Base tiles 64x64 anchored at (0,0), Tx = ceil(W/64), Ty = ceil(H/64).  A node at level
+ * l < 3 with >= 1 in-image pixel splits iff metric(node) > threshold (strict); evaluated
+ * top-down.
+ *   NOIT_QT_VARIANCE: q_c = rint(255 clamp(c,0,1)); split iff
+ *       sum_c (n S2_c - S1_c^2) > var_threshold_q n^2  (exact integers) (A14, A16)
+ *   NOIT_QT_CORNER: D = (1/6) sum over the 6 pairs of the node's 4 in-image corner
+ *       pixels of the Euclidean RGB distance (fp32, fixed order); split iff D > corner_threshold
+ *   tile_mask [Ty*Tx]: bit 0 root; bit 1+c level-1 child c = cx+2cy; bit 5+4c+g level-2 child
+ *   cell_level [ceil(H/8)*ceil(W/8)]: level 0..3 of the leaf containing the 8x8 cell
+ *   level_hist [4] (zeroed by the call): leaves per level with >= 1 in-image pixel    */
+typedef struct {
+    int32_t metric;
+    uint32_t var_threshold_q;      /* summed-over-channels variance, 8-bit units squared      */
+    float corner_threshold;
+} noit_qt_params;
+noit_status noit_quadtree(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t width,
+                          int32_t height, const noit_qt_params* params, uint32_t* tile_mask,
+                          uint8_t* cell_level, uint32_t* level_hist, void* stream);
+
+/* ---- S8 depth-based reprojection with disocclusion test (O8, A21-A23).
+ * Per pixel, fp32 in a fixed order: NDC of the pixel centre and cur_depth -> M -> previous
+ * pixel q and expected depth d_e; accept iff w > 0, q on screen and
+ * |prev_depth[q] - d_e| <= depth_threshold.  Accepted: out_trans[p] = prev_trans[q] (bit
+ * copy), out_depth[p] = d_e, accept[p] = 1, out_final[p] = (C_t + T_tot C_b, 1 - T_tot).
+ * Rejected: accept[p] = 0, p appended to reject_list (order unspecified), outputs untouched.
+ * M = VP_prev * VP_cur^-1, row-major, column vectors.  out_depth/out_final/accept/reject_list
+ * may be NULL; reject_count (required) is zeroed by the call.                                */
+typedef struct {
+    int32_t width, height;
+    float M[16];
+    float depth_threshold;
+    float background[3];
+    const float* prev_trans; const float* prev_depth; const float* cur_depth;
+    float* out_trans; float* out_depth; float* out_final;
+    uint8_t* accept;
+    uint32_t* reject_list; uint32_t* reject_count;
+} noit_reproject_desc;
+noit_status noit_reproject(noit_ctx* ctx, const noit_reproject_desc* desc, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NOIT_H */

@@ -252,7 +252,12 @@ def cfg4(seed: int = 0, W: int = 1920, H: int = 1080, n_prims: int = 512,
     bg.update_bbox()
     allp = _concat(prims, bg)
     full = rasterize(allp, W, H, 1, cap=cap, color_dtype=np.float16, smooth_tiles=smooth)
-    nt = inject_front_ties(full, rng, 0.10)
+    # ties only in the detail tiles: a front tie reorders a pixel's layers, which inside a smooth
+    # region would be salt-and-pepper noise and no 64-px leaf would survive (DESIGN.md recipe)
+    ys = np.minimum(np.arange(H) // 64, Ty - 1)
+    xs = np.minimum(np.arange(W) // 64, Tx - 1)
+    detail_px = ~smooth[ys[:, None], xs[None, :]].reshape(-1)
+    nt = inject_front_ties(full, rng, 0.10, pixel_mask=detail_px)
     half = rasterize(allp, W, H, 2, cap=cap, color_dtype=np.float16, smooth_tiles=smooth)
     quarter = rasterize(allp, W, H, 4, cap=cap, color_dtype=np.float16, smooth_tiles=smooth)
     return Scene("cfg4", full, half, quarter, weights=mlp_weights(seed), mlp_precision=1,

@@ -224,8 +224,12 @@ def rasterize(prims: Primitives, width: int, height: int, r: int = 1, cap: int =
     return FragBuf(Wr, Hr, offsets64.astype(np.uint32), depth, rgba)
 
 
-def inject_front_ties(fb: FragBuf, rng: np.random.Generator, fraction: float) -> int:
+def inject_front_ties(fb: FragBuf, rng: np.random.Generator, fraction: float,
+                      pixel_mask: np.ndarray | None = None) -> int:
     """Give ~`fraction` of the pixels with n_p >= 2 an exact depth tie AT THE FRONT.
+
+    `pixel_mask` (bool [P], optional) restricts the eligible pixels (cfg4: detail tiles only --
+    a tie reorders the layers of a pixel, which in a smooth region is salt-and-pepper noise).
 
     In each chosen pixel the bit pattern of the minimum depth is copied onto one other,
     uniformly chosen fragment of that pixel, so the tie sits on either side of the index order
@@ -235,7 +239,7 @@ def inject_front_ties(fb: FragBuf, rng: np.random.Generator, fraction: float) ->
     off = fb.offsets.astype(np.int64)
     n = np.diff(off)
     P = n.shape[0]
-    cand = np.nonzero(n >= 2)[0]
+    cand = np.nonzero((n >= 2) if pixel_mask is None else ((n >= 2) & pixel_mask))[0]
     if cand.size == 0:
         return 0
     chosen = cand[rng.random(cand.size) < fraction]

@@ -1,0 +1,126 @@
+// noit_api.cu -- context, weights, error reporting and argument checks of libnoit.so.
+#include <stdarg.h>
+
+#include <new>
+
+#include "noit_internal.cuh"
+
+static char g_err[512] = "no error";
+
+noit_status noit_fail(noit_ctx* ctx, noit_status st, const char* fmt, ...)
+{
+    char* dst = ctx ? ctx->err : g_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+noit_status noit_cuda_check(noit_ctx* ctx, cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return NOIT_OK;
+    return noit_fail(ctx, NOIT_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+noit_status noit_check_fragbuf(noit_ctx* ctx, const noit_fragbuf* fb, const char* name)
+{
+    if (!fb) return noit_fail(ctx, NOIT_ERR_NULL, "%s: fragment buffer is NULL", name);
+    if (fb->width <= 0 || fb->height <= 0)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "%s: width/height must be > 0", name);
+    const uint64_t P = (uint64_t)fb->width * (uint64_t)fb->height;
+    if (P + 1 > 0xFFFFFFFFull)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "%s: P+1 overflows u32", name);
+    if (fb->color_fmt != NOIT_RGBA_F16 && fb->color_fmt != NOIT_RGBA_F32)
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: unknown color_fmt %d", name, fb->color_fmt);
+    if (!fb->offsets) return noit_fail(ctx, NOIT_ERR_NULL, "%s: offsets is NULL", name);
+    if (fb->num_fragments > 0 && (!fb->depth || !fb->rgba))
+        return noit_fail(ctx, NOIT_ERR_NULL, "%s: depth/rgba is NULL with F > 0", name);
+    if (!noit_aligned(fb->offsets, 4) || !noit_aligned(fb->depth, 16) ||
+        !noit_aligned(fb->rgba, 16))
+        return noit_fail(ctx, NOIT_ERR_FORMAT,
+                         "%s: offsets need 4-byte, depth/rgba 16-byte alignment", name);
+    return NOIT_OK;
+}
+
+extern "C" {
+
+noit_status noit_create(noit_ctx** out)
+{
+    if (!out) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_create: out is NULL");
+    *out = nullptr;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return noit_cuda_check(nullptr, e, "cudaGetDevice");
+    noit_ctx* c = new (std::nothrow) noit_ctx();
+    if (!c) return noit_fail(nullptr, NOIT_ERR_CUDA, "noit_create: out of host memory");
+    c->device = dev;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+        c->num_sms = sms;
+    e = cudaMalloc(&c->d_counters, 64 * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, 64 * sizeof(uint32_t));
+    if (e != cudaSuccess) {
+        noit_cuda_check(nullptr, e, "noit_create scratch");
+        delete c;
+        return NOIT_ERR_CUDA;
+    }
+    snprintf(c->err, sizeof c->err, "no error");
+    *out = c;
+    return NOIT_OK;
+}
+
+void noit_destroy(noit_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_mlp);
+    cudaFree(ctx->d_coarse_g[0]);
+    cudaFree(ctx->d_coarse_g[1]);
+    cudaFree(ctx->d_stage);
+    delete ctx;
+}
+
+// bf16 round-to-nearest-even of a finite fp32, widened back (A6).
+static float round_bf16(float v)
+{
+    uint32_t u;
+    memcpy(&u, &v, 4);
+    if ((u & 0x7F800000u) != 0x7F800000u) u += 0x7FFFu + ((u >> 16) & 1u);
+    u &= 0xFFFF0000u;
+    memcpy(&v, &u, 4);
+    return v;
+}
+
+noit_status noit_set_weights(noit_ctx* ctx, const float* host_w, int32_t count, int32_t precision)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_set_weights: ctx is NULL");
+    if (!host_w) return noit_fail(ctx, NOIT_ERR_NULL, "noit_set_weights: host_w is NULL");
+    if (count != NOIT_MLP_PARAMS)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_set_weights: count %d != 771 (P:97)", count);
+    if (precision != NOIT_MLP_FP32 && precision != NOIT_MLP_BF16)
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_set_weights: unknown precision %d", precision);
+    float* dst = reinterpret_cast<float*>(&ctx->w);
+    for (int i = 0; i < NOIT_MLP_PARAMS; ++i)
+        dst[i] = precision == NOIT_MLP_BF16 ? round_bf16(host_w[i]) : host_w[i];
+    ctx->precision = precision;
+    ctx->has_weights = true;
+    return NOIT_OK;
+}
+
+noit_status noit_get_weights(const noit_ctx* ctx, float* host_out, int32_t count)
+{
+    noit_ctx* c = const_cast<noit_ctx*>(ctx);
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_get_weights: ctx is NULL");
+    if (!host_out) return noit_fail(c, NOIT_ERR_NULL, "noit_get_weights: host_out is NULL");
+    if (count != NOIT_MLP_PARAMS) return noit_fail(c, NOIT_ERR_SIZE, "noit_get_weights: count != 771");
+    if (!ctx->has_weights) return noit_fail(c, NOIT_ERR_NO_WEIGHTS, "noit_get_weights: no weights set");
+    memcpy(host_out, &ctx->w, sizeof(MlpWeights));
+    return NOIT_OK;
+}
+
+const char* noit_last_error(const noit_ctx* ctx) { return ctx ? ctx->err : g_err; }
+
+uint64_t noit_launch_count(const noit_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,290 @@
+// noit_resolve.cu -- noit_resolve / noit_resolve_host: host-side checks and dispatch, plus the
+// GENERAL resolve kernel (one pixel per thread, fragments read straight from global memory).
+// The general kernel serves S9 (scattered pixel list), S7 (adaptive, per-tile LOD) and any
+// plain frame the staged ring kernel (noit_resolve_ring.cu) does not take.
+#include "noit_resolve_common.cuh"
+
+noit_status noit_launch_resolve_ring(noit_ctx* ctx, const ResolveArgs& A, int color_fmt,
+                                     cudaStream_t st, bool* taken);
+
+enum { MODE_ALL = 0, MODE_LIST = 1, MODE_ADAPTIVE = 2 };
+
+// lod > 0 pixel of S7 (O7): bilinear sample of G = [a2*C2 (3), a2, C_acc (3), A_tail, T_tail, N]
+// at the full-res pixel centre, taps clamped to the coarse texels of the pixel's own leaf and to
+// the image (A19).  lerp(a,b,w) = a + w(b-a), x first then y; the weights are dyadic.
+__device__ __forceinline__ void sample_coarse_g(const float* __restrict__ G, int cw, int ch, int r,
+                                                int leaf_side, int x, int y, float out[10])
+{
+    const float inv_r = 1.f / (float)r;
+    const float u = ((float)x + 0.5f) * inv_r - 0.5f, v = ((float)y + 0.5f) * inv_r - 0.5f;
+    const float fu = floorf(u), fv = floorf(v);
+    const int i0 = (int)fu, j0 = (int)fv;
+    const float wx = u - fu, wy = v - fv;
+    const int lx0 = (x / leaf_side) * leaf_side, ly0 = (y / leaf_side) * leaf_side;
+    const int tx_lo = lx0 / r, ty_lo = ly0 / r;
+    const int tx_hi = min((lx0 + leaf_side - 1) / r, cw - 1);
+    const int ty_hi = min((ly0 + leaf_side - 1) / r, ch - 1);
+    const int xa = min(max(i0, tx_lo), tx_hi), xb = min(max(i0 + 1, tx_lo), tx_hi);
+    const int ya = min(max(j0, ty_lo), ty_hi), yb = min(max(j0 + 1, ty_lo), ty_hi);
+    const float* g00 = G + 10 * ((size_t)ya * cw + xa);
+    const float* g10 = G + 10 * ((size_t)ya * cw + xb);
+    const float* g01 = G + 10 * ((size_t)yb * cw + xa);
+    const float* g11 = G + 10 * ((size_t)yb * cw + xb);
+#pragma unroll
+    for (int k = 0; k < 10; ++k) {
+        const float a = g00[k], b = g10[k], c = g01[k], d = g11[k];
+        const float top = fmaf(wx, b - a, a), bot = fmaf(wx, d - c, c);
+        out[k] = fmaf(wy, bot - top, top);
+    }
+}
+
+template <typename ColorT, int kMode>
+__global__ void __launch_bounds__(128)
+resolve_general_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeights W)
+{
+    const ColorT* __restrict__ rgba = static_cast<const ColorT*>(A.rgba);
+    const uint32_t stride = gridDim.x * blockDim.x;
+    const uint32_t total = kMode == MODE_LIST ? min(__ldg(A.pixel_count), A.P) : A.P;
+    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += stride) {
+        const uint32_t p = kMode == MODE_LIST ? __ldg(A.pixel_list + t) : t;
+        const uint32_t b = __ldg(A.offsets + p), e = __ldg(A.offsets + p + 1);
+        int lod = 0, level = 3, x = 0, y = 0;
+        if (kMode == MODE_ADAPTIVE) {
+            y = (int)(p / (uint32_t)A.W);
+            x = (int)(p - (uint32_t)y * (uint32_t)A.W);
+            level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)];
+            lod = A.level_to_lod[level & 3];
+        }
+        float xf[5], f[3];
+        if (kMode != MODE_ADAPTIVE || lod == 0) {
+            PixelState<false> s;
+            s.init();
+            for (uint32_t j = b; j < e; ++j) s.push(__ldg(A.depth + j), load_rgba(rgba, j), j);
+            const bool has_tail = make_features((float)(e - b), s.t_tail, s.acc_r, s.acc_g,
+                                                s.acc_b, s.a_tail, xf);
+            mlp_forward(W, xf, f);
+            const float4 l2 = make_float4(s.c2.w * s.c2.x, s.c2.w * s.c2.y, s.c2.w * s.c2.z, s.c2.w);
+            composite_store(A, p, s.c1, l2, e > b ? s.d1 : 1.0f, has_tail, f, s.t_tail);
+        } else {
+            // layer 1 from the FULL buffer: depth-only scan, then one colour fetch
+            float d1 = __int_as_float(0x7f800000);
+            uint32_t i1 = b;
+            for (uint32_t j = b; j < e; ++j) {
+                const float d = __ldg(A.depth + j);
+                if (d < d1) { d1 = d; i1 = j; }
+            }
+            float4 c1 = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (e > b) c1 = load_rgba(rgba, i1); else d1 = 1.0f;
+            float G[10];
+            sample_coarse_g(A.coarse_g[lod - 1], A.coarse_w[lod - 1], A.coarse_h[lod - 1], 1 << lod,
+                            64 >> level, x, y, G);
+            const bool has_tail = make_features(G[9], G[8], G[4], G[5], G[6], G[7], xf);
+            mlp_forward(W, xf, f);
+            composite_store(A, p, c1, make_float4(G[0], G[1], G[2], G[3]), d1, has_tail, f, G[8]);
+        }
+    }
+}
+
+// S7 pre-pass: G[10] of every coarse pixel whose leaf is resolved at this lod (self-contained
+// O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
+template <typename ColorT>
+__global__ void __launch_bounds__(128)
+coarse_g_kernel(int cw, int ch, int r, int lod, int full_w, const uint8_t* __restrict__ cell_level,
+                uchar4 level_to_lod, const uint32_t* __restrict__ offsets,
+                const float* __restrict__ depth, const ColorT* __restrict__ rgba,
+                float* __restrict__ G)
+{
+    const uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= (uint32_t)cw * (uint32_t)ch) return;
+    const int Y = q / cw, X = q - Y * cw;
+    const int level = cell_level[(size_t)((Y * r) >> 3) * ((full_w + 7) >> 3) + ((X * r) >> 3)] & 3;
+    const uint8_t l2l[4] = {level_to_lod.x, level_to_lod.y, level_to_lod.z, level_to_lod.w};
+    if (l2l[level] != lod) return;
+    const uint32_t b = __ldg(offsets + q), e = __ldg(offsets + q + 1);
+    PixelState<false> s;
+    s.init();
+    for (uint32_t j = b; j < e; ++j) s.push(__ldg(depth + j), load_rgba(rgba, j), j);
+    float* g = G + 10 * (size_t)q;
+    g[0] = s.c2.w * s.c2.x; g[1] = s.c2.w * s.c2.y; g[2] = s.c2.w * s.c2.z; g[3] = s.c2.w;
+    g[4] = s.acc_r; g[5] = s.acc_g; g[6] = s.acc_b; g[7] = s.a_tail; g[8] = s.t_tail;
+    g[9] = (float)(e - b);
+}
+
+// ------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------
+static noit_status check_desc(noit_ctx* ctx, const noit_resolve_desc* d, const char* who)
+{
+    if (!d) return noit_fail(ctx, NOIT_ERR_NULL, "%s: desc is NULL", who);
+    NOIT_TRY(noit_check_fragbuf(ctx, &d->full, who));
+    if (!ctx->has_weights) return noit_fail(ctx, NOIT_ERR_NO_WEIGHTS, "%s: no weights set", who);
+    if (!d->out_trans && !d->out_final && !d->out_depth1)
+        return noit_fail(ctx, NOIT_ERR_NULL, "%s: every output is NULL", who);
+    if (!noit_aligned(d->out_trans, 16) || !noit_aligned(d->out_final, 16) ||
+        !noit_aligned(d->out_depth1, 4))
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: out_trans/out_final need 16-byte alignment", who);
+    if ((d->pixel_list != nullptr) != (d->pixel_count != nullptr))
+        return noit_fail(ctx, NOIT_ERR_NULL, "%s: pixel_list and pixel_count go together", who);
+    if (d->pixel_list && d->cell_level)
+        return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "%s: pixel_list with cell_level", who);
+    if (d->cell_level) {
+        for (int l = 0; l < 4; ++l) {
+            const int lod = d->level_to_lod[l];
+            if (lod > 2) return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: level_to_lod[%d] > 2", who, l);
+            const noit_fragbuf* cb = lod == 1 ? d->half : (lod == 2 ? d->quarter : nullptr);
+            if (lod == 0) continue;
+            if (!cb) return noit_fail(ctx, NOIT_ERR_NULL, "%s: lod %d buffer is NULL", who, lod);
+            NOIT_TRY(noit_check_fragbuf(ctx, cb, who));
+            const int r = 1 << lod;
+            if (cb->width != (d->full.width + r - 1) / r || cb->height != (d->full.height + r - 1) / r)
+                return noit_fail(ctx, NOIT_ERR_SIZE, "%s: lod %d buffer is not ceil(W/%d) x ceil(H/%d)",
+                                 who, lod, r, r);
+            if (cb->color_fmt != d->full.color_fmt)
+                return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: coarse buffers must share color_fmt", who);
+        }
+    }
+    return NOIT_OK;
+}
+
+template <int kMode>
+static void launch_general(const ResolveArgs& A, const MlpWeights& W, int fmt, uint32_t blocks,
+                           cudaStream_t st)
+{
+    if (fmt == NOIT_RGBA_F16)
+        resolve_general_kernel<__half, kMode><<<blocks, 128, 0, st>>>(A, W);
+    else
+        resolve_general_kernel<float, kMode><<<blocks, 128, 0, st>>>(A, W);
+}
+
+static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cudaStream_t st)
+{
+    ResolveArgs A;
+    memset(&A, 0, sizeof A);
+    A.W = d->full.width;
+    A.H = d->full.height;
+    A.P = (uint32_t)A.W * (uint32_t)A.H;
+    A.offsets = d->full.offsets;
+    A.depth = d->full.depth;
+    A.rgba = d->full.rgba;
+    memcpy(A.bg, d->background, sizeof A.bg);
+    A.out_trans = d->out_trans;
+    A.out_final = d->out_final;
+    A.out_depth1 = d->out_depth1;
+    A.pixel_list = d->pixel_list;
+    A.pixel_count = d->pixel_count;
+    A.cell_level = d->cell_level;
+    const int fmt = d->full.color_fmt;
+
+    if (d->pixel_list) {                                   // S9
+        launch_general<MODE_LIST>(A, ctx->w, fmt, (uint32_t)ctx->num_sms * 8, st);
+        ctx->launches += 1;
+        NOIT_CUDA(ctx, cudaGetLastError());
+        return NOIT_OK;
+    }
+    if (d->cell_level) {                                   // S7
+        memcpy(A.level_to_lod, d->level_to_lod, 4);
+        const uchar4 l2l = make_uchar4(d->level_to_lod[0], d->level_to_lod[1], d->level_to_lod[2],
+                                       d->level_to_lod[3]);
+        for (int lod = 1; lod <= 2; ++lod) {
+            bool used = false;
+            for (int l = 0; l < 4; ++l) used |= d->level_to_lod[l] == lod;
+            if (!used) continue;
+            const noit_fragbuf* cb = lod == 1 ? d->half : d->quarter;
+            const size_t cp = (size_t)cb->width * cb->height;
+            if (ctx->coarse_g_cap[lod - 1] < cp) {
+                if (ctx->d_coarse_g[lod - 1]) {
+                    NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+                    NOIT_CUDA(ctx, cudaFree(ctx->d_coarse_g[lod - 1]));
+                    ctx->d_coarse_g[lod - 1] = nullptr;
+                    ctx->coarse_g_cap[lod - 1] = 0;
+                }
+                NOIT_CUDA(ctx, cudaMalloc(&ctx->d_coarse_g[lod - 1], cp * 10 * sizeof(float)));
+                ctx->coarse_g_cap[lod - 1] = cp;
+            }
+            A.coarse_g[lod - 1] = ctx->d_coarse_g[lod - 1];
+            A.coarse_w[lod - 1] = cb->width;
+            A.coarse_h[lod - 1] = cb->height;
+            const uint32_t blocks = (uint32_t)((cp + 127) / 128);
+            if (fmt == NOIT_RGBA_F16)
+                coarse_g_kernel<__half><<<blocks, 128, 0, st>>>(
+                    cb->width, cb->height, 1 << lod, lod, A.W, d->cell_level, l2l, cb->offsets,
+                    cb->depth, (const __half*)cb->rgba, ctx->d_coarse_g[lod - 1]);
+            else
+                coarse_g_kernel<float><<<blocks, 128, 0, st>>>(
+                    cb->width, cb->height, 1 << lod, lod, A.W, d->cell_level, l2l, cb->offsets,
+                    cb->depth, (const float*)cb->rgba, ctx->d_coarse_g[lod - 1]);
+            ctx->launches += 1;
+            NOIT_CUDA(ctx, cudaGetLastError());
+        }
+        launch_general<MODE_ADAPTIVE>(A, ctx->w, fmt, (A.P + 127) / 128, st);
+        ctx->launches += 1;
+        NOIT_CUDA(ctx, cudaGetLastError());
+        return NOIT_OK;
+    }
+    bool taken = false;                                    // plain frame: staged ring kernel
+    NOIT_TRY(noit_launch_resolve_ring(ctx, A, fmt, st, &taken));
+    if (!taken) {
+        launch_general<MODE_ALL>(A, ctx->w, fmt, (A.P + 127) / 128, st);
+        ctx->launches += 1;
+        NOIT_CUDA(ctx, cudaGetLastError());
+    }
+    return NOIT_OK;
+}
+
+extern "C" {
+
+noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* d, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve: ctx is NULL");
+    NOIT_TRY(check_desc(ctx, d, "noit_resolve"));
+    return resolve_device(ctx, d, (cudaStream_t)stream);
+}
+
+noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve_host: ctx is NULL");
+    if (h && (h->cell_level || h->pixel_list || h->half || h->quarter))
+        return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "noit_resolve_host: plain resolve only");
+    NOIT_TRY(check_desc(ctx, h, "noit_resolve_host"));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t P = (size_t)h->full.width * h->full.height, F = h->full.num_fragments;
+    const size_t cb = h->full.color_fmt == NOIT_RGBA_F16 ? 8 : 16;
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t o_off = 0, o_depth = o_off + up(4 * (P + 1)), o_rgba = o_depth + up(4 * F);
+    const size_t o_trans = o_rgba + up(cb * F), o_final = o_trans + up(16 * P);
+    const size_t o_d1 = o_final + up(16 * P), total = o_d1 + up(4 * P);
+    if (ctx->stage_cap < total) {
+        if (ctx->d_stage) {
+            NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+            NOIT_CUDA(ctx, cudaFree(ctx->d_stage));
+            ctx->d_stage = nullptr;
+            ctx->stage_cap = 0;
+        }
+        NOIT_CUDA(ctx, cudaMalloc(&ctx->d_stage, total));
+        ctx->stage_cap = total;
+    }
+    char* base = static_cast<char*>(ctx->d_stage);
+    NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_off, h->full.offsets, 4 * (P + 1), cudaMemcpyHostToDevice, st));
+    if (F) {
+        NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_depth, h->full.depth, 4 * F, cudaMemcpyHostToDevice, st));
+        NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_rgba, h->full.rgba, cb * F, cudaMemcpyHostToDevice, st));
+    }
+    noit_resolve_desc d = *h;
+    d.full.offsets = reinterpret_cast<const uint32_t*>(base + o_off);
+    d.full.depth = reinterpret_cast<const float*>(base + o_depth);
+    d.full.rgba = base + o_rgba;
+    d.out_trans = h->out_trans ? reinterpret_cast<float*>(base + o_trans) : nullptr;
+    d.out_final = h->out_final ? reinterpret_cast<float*>(base + o_final) : nullptr;
+    d.out_depth1 = h->out_depth1 ? reinterpret_cast<float*>(base + o_d1) : nullptr;
+    NOIT_TRY(resolve_device(ctx, &d, st));
+    if (h->out_trans)
+        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_trans, d.out_trans, 16 * P, cudaMemcpyDeviceToHost, st));
+    if (h->out_final)
+        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_final, d.out_final, 16 * P, cudaMemcpyDeviceToHost, st));
+    if (h->out_depth1)
+        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_depth1, d.out_depth1, 4 * P, cudaMemcpyDeviceToHost, st));
+    NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+    return NOIT_OK;
+}
+
+}  // extern "C"

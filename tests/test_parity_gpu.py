@@ -1,0 +1,227 @@
+"""GPU parity (`-m gpu`): the CUDA path through the C ABI versus the CPU oracle, element by
+element on the same seeded inputs.  Classes:
+  bit-exact  : idx1, idx2, count, depth1, tile_mask, cell_level, hist, accept, reject set,
+               reprojected copies
+  fp32       : |a-b| <= 1e-5 max(|a|,|b|) + 1e-6   (layers, tail accumulators, compositing)
+  mlp-fp32   : the above + 1e-5 * T_2 * mag(f), mag(f) = the MLP evaluated with |W|, |b|, |x|
+               (forward error bound of fp32 dot products with cancellation)
+  bf16 mode  : 2e-3 absolute on colour (BASELINE.json north_star)
+"""
+import numpy as np
+import pytest
+import torch
+
+import noit_scenes
+import oracle
+from noit_scenes.raster import FragBuf
+
+pytestmark = pytest.mark.gpu
+BG = (0.2, 0.3, 0.4)
+
+
+@pytest.fixture(scope="module")
+def noit():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_16747_b200 as m
+    return m
+
+
+def close(a, b, rel=1e-5, abs_=1e-6, extra=None):
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    tol = rel * np.maximum(np.abs(a), np.abs(b)) + abs_
+    if extra is not None:
+        tol = tol + extra
+    bad = np.abs(a - b) > tol
+    if bad.any():
+        i = np.argwhere(bad)[0]
+        raise AssertionError(f"{bad.sum()} mismatches, first at {tuple(i)}: {a[tuple(i)]} vs {b[tuple(i)]}")
+    return True
+
+
+def u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def mlp_magnitude(w_eff, feats):
+    """|W3|(|W2|(|W1||x|+|b1|)+|b2|)+|b3| in float64: scale of the rounding error of f(x)."""
+    w = np.abs(w_eff.astype(np.float64))
+    W1, b1 = w[:160].reshape(32, 5), w[160:192]
+    W2, b2 = w[192:704].reshape(16, 32), w[704:720]
+    W3, b3 = w[720:768].reshape(3, 16), w[768:771]
+    x = np.abs(feats.astype(np.float64))
+    return ((x @ W1.T + b1) @ W2.T + b2) @ W3.T + b3
+
+
+def check_resolve(noit, fb_host, weights, precision, got, ref=None, bf16_abs=2e-3):
+    w_eff = oracle.effective_weights(weights, precision)
+    if ref is None:
+        ref = oracle.resolve(fb_host, w_eff, BG)
+    lay = oracle.build_features(fb_host)
+    a1, a2 = lay["layer1"][:, 3].astype(np.float64), lay["layer2"][:, 3].astype(np.float64)
+    t2 = (1 - a1) * (1 - a2)
+    mag = mlp_magnitude(w_eff, lay["features"]) * t2[:, None]
+    extra = np.concatenate([1e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])          # bit-exact
+    for k in ("trans", "final"):
+        g = got[k].cpu().numpy()
+        close(g, ref[k], extra=extra)
+        if precision == 1:                       # BASELINE.json: 2e-3 absolute on colour
+            assert np.max(np.abs(g[:, :3].astype(np.float64) - ref[k][:, :3])) <= bf16_abs
+    return ref
+
+
+def random_fb(rng, W, H, max_n, dtype, tie_frac=0.3, empty_frac=0.2, heavy=None):
+    P = W * H
+    counts = rng.integers(0, max_n + 1, P)
+    counts[rng.random(P) < empty_frac] = 0
+    if heavy:
+        counts[rng.integers(0, P, heavy[0])] = heavy[1]
+    off = np.zeros(P + 1, np.uint32)
+    off[1:] = np.cumsum(counts)
+    F = int(off[-1])
+    depth = rng.uniform(0.01, 0.99, F).astype(np.float32)
+    ties = rng.random(F) < tie_frac
+    depth[ties] = rng.choice(np.asarray([0.25, 0.5, 0.75], np.float32), int(ties.sum()))
+    rgba = rng.uniform(0, 1, (F, 4)).astype(dtype)
+    return FragBuf(W, H, off, depth, rgba)
+
+
+# -------------------------------------------------------------------------------------------
+# S1-S3
+# -------------------------------------------------------------------------------------------
+def check_layers(noit, fb_host):
+    ctx = noit.Noit()
+    got = ctx.build_features(noit.DeviceFragBuf.from_host(fb_host))
+    ref = oracle.build_features(fb_host)
+    for k in ("idx1", "idx2", "count"):
+        assert np.array_equal(u32(got[k]), ref[k]), k
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    assert np.array_equal(got["layer1"].cpu().numpy(), ref["layer1"])          # exact copies
+    assert np.array_equal(got["layer2"].cpu().numpy(), ref["layer2"])
+    close(got["tail_raw"].cpu().numpy(), ref["tail_raw"])
+    close(got["features"].cpu().numpy(), ref["features"])
+
+
+def test_build_features_cfg1(noit, cfg1_scene):
+    check_layers(noit, cfg1_scene.full)
+
+
+@pytest.mark.parametrize("dtype,seed", [(np.float32, 1), (np.float16, 2)])
+def test_build_features_random_ties(noit, dtype, seed):
+    rng = np.random.default_rng(seed)
+    check_layers(noit, random_fb(rng, 67, 45, 12, dtype, tie_frac=0.5))
+
+
+def test_build_features_heavy_and_empty(noit):
+    rng = np.random.default_rng(3)
+    check_layers(noit, random_fb(rng, 50, 21, 6, np.float16, heavy=(20, 300)))
+    empty = FragBuf(5, 3, np.zeros(16, np.uint32), np.zeros(0, np.float32), np.zeros((0, 4), np.float16))
+    check_layers(noit, empty)
+
+
+# -------------------------------------------------------------------------------------------
+# S4
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [0, 1])
+def test_infer(noit, precision):
+    rng = np.random.default_rng(4)
+    w = noit_scenes.mlp_weights(7)
+    n = 10007
+    x = np.concatenate([rng.integers(0, 129, (n, 1)).astype(np.float32),
+                        rng.random((n, 4)).astype(np.float32)], axis=1)
+    ctx = noit.Noit(w, precision)
+    w_eff = oracle.effective_weights(w, precision)
+    assert np.array_equal(ctx.get_weights(), w_eff)                  # same rounding, bit for bit
+    got = ctx.infer(torch.from_numpy(x).cuda()).cpu().numpy()
+    close(got, oracle.infer(w_eff, x), extra=1e-5 * mlp_magnitude(w_eff, x))
+    assert ctx.infer(torch.empty((0, 5), device="cuda")).shape == (0, 3)
+
+
+# -------------------------------------------------------------------------------------------
+# S1-S5 fused
+# -------------------------------------------------------------------------------------------
+def test_resolve_cfg1(noit, cfg1_scene):
+    sc = cfg1_scene
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(sc.full), BG)
+    check_resolve(noit, sc.full, sc.weights, sc.mlp_precision, got)
+
+
+@pytest.mark.parametrize("dtype,precision,seed,shape", [
+    (np.float32, 0, 11, (67, 45)), (np.float16, 1, 12, (130, 33)), (np.float16, 0, 13, (31, 7)),
+    (np.float16, 1, 14, (1, 1)), (np.float32, 1, 15, (257, 3))])
+def test_resolve_random_ragged(noit, dtype, precision, seed, shape):
+    rng = np.random.default_rng(seed)
+    fbh = random_fb(rng, shape[0], shape[1], 40, dtype, heavy=(5, 700))
+    w = noit_scenes.mlp_weights(seed)
+    ctx = noit.Noit(w, precision)
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
+    check_resolve(noit, fbh, w, precision, got)
+
+
+def test_resolve_empty_and_single_output(noit):
+    w = noit_scenes.mlp_weights(0)
+    ctx = noit.Noit(w, 0)
+    empty = FragBuf(40, 3, np.zeros(121, np.uint32), np.zeros(0, np.float32), np.zeros((0, 4), np.float16))
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(empty), BG)
+    assert torch.all(got["trans"] == torch.tensor([0, 0, 0, 1.0], device="cuda"))
+    assert torch.all(got["final"] == torch.tensor([BG[0], BG[1], BG[2], 0.0], device="cuda"))
+    assert torch.all(got["depth1"] == 1.0)
+    rng = np.random.default_rng(5)
+    fbh = random_fb(rng, 64, 9, 10, np.float16)
+    full = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
+    only = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG, want=("final",))
+    assert set(only) == {"final"} and torch.equal(only["final"], full["final"])
+
+
+def test_resolve_empty_tail_is_exact_two_layer_composite(noit):
+    """BASELINE.json invariant on the GPU path: n_p <= 2 => output == Eq. 1 on the fragments."""
+    rng = np.random.default_rng(6)
+    fbh = random_fb(rng, 96, 20, 2, np.float32, empty_frac=0.1)
+    ctx = noit.Noit(noit_scenes.mlp_weights(1), 0)
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)["final"].cpu().numpy()
+    close(got, oracle.exact(fbh, BG)["final"])
+
+
+@pytest.fixture(scope="module")
+def cfg2_scene():
+    return noit_scenes.cfg2(0)
+
+
+@pytest.fixture(scope="module")
+def cfg3_scene():
+    return noit_scenes.cfg3(0)
+
+
+def test_resolve_cfg2_full(noit, cfg2_scene):
+    sc = cfg2_scene
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(sc.full), BG)
+    check_resolve(noit, sc.full, sc.weights, sc.mlp_precision, got)
+
+
+def test_resolve_cfg3_full_and_layers(noit, cfg3_scene):
+    """BASELINE.json's 1080p config at FULL size, element by element (the oracle needs ~1 s)."""
+    sc = cfg3_scene
+    fb = noit.DeviceFragBuf.from_host(sc.full)
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    got = ctx.resolve(fb, BG)
+    check_resolve(noit, sc.full, sc.weights, sc.mlp_precision, got)
+    lay = ctx.build_features(fb, want=("idx1", "idx2", "count"))
+    ref = oracle.build_features(sc.full)
+    for k in ("idx1", "idx2", "count"):
+        assert np.array_equal(u32(lay[k]), ref[k]), k
+    assert sc.meta["tie_pixels"] > 0.05 * sc.full.num_pixels
+
+
+def test_resolve_host_matches_device(noit, cfg1_scene):
+    sc = cfg1_scene
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    dev = ctx.resolve(noit.DeviceFragBuf.from_host(sc.full), BG)
+    P = sc.full.num_pixels
+    trans, final, d1 = (np.zeros((P, 4), np.float32), np.zeros((P, 4), np.float32), np.zeros(P, np.float32))
+    ctx.resolve_host(sc.full, BG, trans, final, d1)
+    assert np.array_equal(trans, dev["trans"].cpu().numpy())
+    assert np.array_equal(final, dev["final"].cpu().numpy())
+    assert np.array_equal(d1, dev["depth1"].cpu().numpy())

@@ -1,0 +1,249 @@
+"""GPU parity for the adjacent steps (`-m gpu`): S6 quadtree, S7 adaptive resolve, S8
+reprojection, S9 fallback resolve, and the ABI's error behaviour."""
+import numpy as np
+import pytest
+import torch
+
+import noit_scenes
+import oracle
+from test_parity_gpu import BG, check_resolve, close, mlp_magnitude, noit, random_fb, u32  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def qt_equal(got, ref):
+    assert np.array_equal(u32(got["tile_mask"]), ref["tile_mask"])
+    assert np.array_equal(got["cell_level"].cpu().numpy(), ref["cell_level"])
+    assert np.array_equal(u32(got["hist"]), ref["hist"])
+
+
+# -------------------------------------------------------------------------------------------
+# S6
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("W,H", [(64, 64), (200, 136), (1920, 1080), (65, 7)])
+@pytest.mark.parametrize("metric", [0, 1])
+def test_quadtree_random_images(noit, W, H, metric):
+    rng = np.random.default_rng(W * 7 + H + metric)
+    # smooth field + blocks of noise so that every level of the tree occurs
+    yy, xx = np.mgrid[0:H, 0:W]
+    img = np.zeros((H, W, 4), np.float32)
+    for c in range(3):
+        img[..., c] = 0.5 + 0.3 * np.sin(xx / (40.0 + 10 * c)) * np.cos(yy / 55.0)
+    noise = rng.random((H, W, 3)).astype(np.float32)
+    sel = (rng.random((-(-H // 16), -(-W // 16))) < 0.3).repeat(16, 0).repeat(16, 1)[:H, :W]
+    amp = rng.choice([0.0, 0.02, 0.3], size=sel.shape).astype(np.float32)
+    img[..., :3] += (sel * amp)[..., None] * (noise - 0.5)
+    img[..., :3] += (rng.random((H, W, 3)) < 0.001) * 2.0 - (rng.random((H, W, 3)) < 0.001) * 2.0
+    img[..., 3] = rng.random((H, W))
+    img = np.ascontiguousarray(img.reshape(-1, 4))
+    ctx = noit.Noit()
+    for thr, cthr in ((6, 0.02), (0, 0.0), (400, 0.2)):
+        got = ctx.quadtree(torch.from_numpy(img).cuda(), W, H, metric, thr, cthr)
+        ref = oracle.quadtree(img, W, H, metric, thr, cthr)
+        qt_equal(got, ref)
+    levels = set(np.unique(oracle.quadtree(img, W, H, metric, 6, 0.02)["cell_level"]).tolist())
+    if W >= 200:
+        assert levels == {0, 1, 2, 3} or metric == 1
+
+
+def test_quadtree_constant_image(noit):
+    W, H = 300, 200
+    img = np.tile(np.asarray([0.3, 0.6, 0.9, 1.0], np.float32), (W * H, 1))
+    got = noit.Noit().quadtree(torch.from_numpy(img).cuda(), W, H)
+    assert int(got["tile_mask"].abs().sum()) == 0
+    assert u32(got["hist"]).tolist() == [5 * 4, 0, 0, 0]
+
+
+def test_quadtree_on_resolved_cfg1(noit, cfg1_scene):
+    sc = cfg1_scene
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    final = ctx.resolve(noit.DeviceFragBuf.from_host(sc.full), BG)["final"]
+    for metric in (0, 1):
+        got = ctx.quadtree(final, 64, 64, metric, 6, 0.02)
+        qt_equal(got, oracle.quadtree(final.cpu().numpy(), 64, 64, metric, 6, 0.02))   # same image (A16)
+
+
+# -------------------------------------------------------------------------------------------
+# S7
+# -------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def cfg4_small():
+    return noit_scenes.cfg4(0, W=448, H=264, n_prims=96, mean_band=(10.0, 12.0), cap=64)
+
+
+def run_adaptive(noit, sc, l2l=(2, 1, 0, 0), thr=6):
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    plain = ctx.resolve(fb, BG)
+    qt = ctx.quadtree(plain["final"], fb.width, fb.height, 0, thr)
+    got = ctx.resolve(fb, BG, half=hb, quarter=qb, cell_level=qt["cell_level"], level_to_lod=l2l)
+    cell = qt["cell_level"].cpu().numpy()
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    ref = oracle.resolve(sc.full, w_eff, BG, half=sc.half, quarter=sc.quarter, cell_level=cell,
+                         level_to_lod=l2l)
+    return plain, got, ref, cell
+
+
+def test_adaptive_resolve_small(noit, cfg4_small):
+    sc = cfg4_small
+    plain, got, ref, cell = run_adaptive(noit, sc)
+    assert {0, 1}.issubset(set(np.unique(cell).tolist())) or 0 in cell      # coarse leaves exist
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    # features of coarse pixels are interpolated: bound the MLP error with a generous magnitude
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    lay = oracle.build_features(sc.full)
+    mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=extra)
+        assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
+    # all levels -> lod 0 is bitwise the plain resolve
+    _, got0, _, _ = run_adaptive(noit, sc, l2l=(0, 0, 0, 0))
+    for k in ("trans", "final", "depth1"):
+        assert torch.equal(got0[k], plain[k]), k
+
+
+def test_adaptive_all_coarse(noit, cfg4_small):
+    """Force every leaf coarse (huge threshold => all 64-leaves => quarter res everywhere)."""
+    sc = cfg4_small
+    _, got, ref, cell = run_adaptive(noit, sc, thr=10 ** 9)
+    assert set(np.unique(cell).tolist()) == {0}
+    for k in ("trans", "final"):
+        assert np.max(np.abs(got[k].cpu().numpy() - ref[k])) <= 2e-3
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+
+
+# -------------------------------------------------------------------------------------------
+# S8 / S9
+# -------------------------------------------------------------------------------------------
+def rand_prev(rng, W, H):
+    P = W * H
+    return (rng.random((P, 4)).astype(np.float32), rng.uniform(0.05, 0.95, P).astype(np.float32))
+
+
+def check_reproject(noit, W, H, M, thr, prev_t, prev_d, cur_d):
+    ctx = noit.Noit()
+    got = ctx.reproject(W, H, M, thr, BG, torch.from_numpy(prev_t).cuda(), torch.from_numpy(prev_d).cuda(),
+                        torch.from_numpy(cur_d).cuda())
+    ref = oracle.reproject(W, H, M, thr, BG, prev_t, prev_d, cur_d)
+    acc = got["accept"].cpu().numpy()
+    assert np.array_equal(acc, ref["accept"])                                  # bit-exact mask
+    n = int(got["reject_count"].item())
+    assert n == ref["reject_count"]
+    assert np.array_equal(np.sort(u32(got["reject_list"])[:n]), np.sort(ref["reject_list"]))
+    m = acc.astype(bool)
+    assert np.array_equal(got["trans"].cpu().numpy()[m], ref["trans"][m])      # bit copies
+    assert np.array_equal(got["depth"].cpu().numpy()[m], ref["depth"][m])
+    close(got["final"].cpu().numpy()[m], ref["final"][m])
+    assert not got["trans"].cpu().numpy()[~m].any()                            # rejected: untouched
+    return got, ref
+
+
+def test_reproject_identity_and_shift(noit):
+    rng = np.random.default_rng(21)
+    W, H = 333, 77
+    prev_t, prev_d = rand_prev(rng, W, H)
+    got, _ = check_reproject(noit, W, H, np.eye(4, dtype=np.float32), 1e-3, prev_t, prev_d, prev_d)
+    assert int(got["reject_count"].item()) == 0
+    assert np.array_equal(got["trans"].cpu().numpy(), prev_t)
+    M = np.eye(4, dtype=np.float32)
+    M[0, 3] = 2.0 * 5 / W                                                      # 5-pixel NDC shift
+    got, ref = check_reproject(noit, W, H, M, 2.0, prev_t, prev_d, prev_d)
+    assert ref["reject_count"] >= 4 * H
+
+
+def test_reproject_perspective_path(noit):
+    rng = np.random.default_rng(22)
+    W, H = 640, 360
+    proj = noit_scenes.perspective(60.0, W / H, 0.1, 100.0)
+    vp0 = proj @ noit_scenes.view_matrix(np.zeros(3), 0.0, 0.0)
+    vp1 = proj @ noit_scenes.view_matrix(np.asarray([0.05, -0.02, 0.03]), 0.004, -0.003)
+    M = (vp0 @ np.linalg.inv(vp1)).astype(np.float32)
+    prev_t, _ = rand_prev(rng, W, H)
+    yy, xx = np.mgrid[0:H, 0:W]
+    prev_d = (0.97 + 0.02 * np.sin(xx / 50.0) * np.cos(yy / 40.0)).astype(np.float32).reshape(-1)
+    prev_d[rng.random(W * H) < 0.05] = 1.0
+    got, ref = check_reproject(noit, W, H, M, 1e-3, prev_t, prev_d, prev_d)
+    frac = ref["reject_count"] / (W * H)
+    assert 0.0 < frac < 1.0
+    Mneg = M.copy()
+    Mneg[3] = -Mneg[3]                                                         # w <= 0 everywhere
+    got, ref = check_reproject(noit, W, H, Mneg, 1e-3, prev_t, prev_d, prev_d)
+    assert ref["reject_count"] == W * H
+
+
+def test_fallback_resolve_on_reject_list(noit):
+    """S8 + S9: union of accepted and re-resolved pixels covers the frame exactly once; with a
+    negative threshold everything is rejected and the frame equals the plain resolve bitwise."""
+    rng = np.random.default_rng(23)
+    W, H = 160, 96
+    fbh = random_fb(rng, W, H, 24, np.float16)
+    w = noit_scenes.mlp_weights(3)
+    ctx = noit.Noit(w, 1)
+    fb = noit.DeviceFragBuf.from_host(fbh)
+    plain = ctx.resolve(fb, BG)
+    M = np.eye(4, dtype=np.float32)
+    M[0, 3] = 2.0 * 3 / W
+    for thr in (0.05, -1.0):
+        rp = ctx.reproject(W, H, M, thr, BG, plain["trans"], plain["depth1"], plain["depth1"])
+        out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+        ctx.resolve(fb, BG, out=out, pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
+        acc = rp["accept"].cpu().numpy().astype(bool)
+        n = int(rp["reject_count"].item())
+        assert n == int((~acc).sum())
+        w_eff = oracle.effective_weights(w, 1)
+        ref_rp = oracle.reproject(W, H, M, thr, BG, plain["trans"].cpu().numpy(),
+                                  plain["depth1"].cpu().numpy(), plain["depth1"].cpu().numpy())
+        ref = dict(trans=ref_rp["trans"], final=ref_rp["final"], depth1=ref_rp["depth"])
+        oracle.resolve(fbh, w_eff, BG, pixel_list=ref_rp["reject_list"], out=ref)
+        for k in ("trans", "final"):
+            assert np.max(np.abs(out[k].cpu().numpy() - ref[k])) <= 2e-3
+        for k in ("trans", "final", "depth1"):                                 # rejected == plain
+            assert torch.equal(out[k][~torch.from_numpy(acc).cuda()], plain[k][~torch.from_numpy(acc).cuda()])
+        if thr < 0:
+            assert n == W * H
+            for k in ("trans", "final", "depth1"):
+                assert torch.equal(out[k], plain[k])
+
+
+# -------------------------------------------------------------------------------------------
+# ABI error behaviour: host-checkable errors come back before any launch
+# -------------------------------------------------------------------------------------------
+def test_abi_errors(noit, cfg1_scene):
+    import ctypes as C
+    sc = cfg1_scene
+    fb = noit.DeviceFragBuf.from_host(sc.full)
+    ctx = noit.Noit()
+    with pytest.raises(noit.NoitError) as e:
+        ctx.resolve(fb, BG)
+    assert e.value.status == 4                                   # NOIT_ERR_NO_WEIGHTS
+    with pytest.raises(noit.NoitError) as e:
+        ctx.set_weights(np.zeros(770, np.float32))
+    assert e.value.status == 2
+    with pytest.raises(noit.NoitError) as e:
+        ctx.set_weights(sc.weights, 7)
+    assert e.value.status == 3
+    ctx.set_weights(sc.weights, 0)
+    L = noit.lib()
+    assert L.noit_resolve(None, None, None) == 1
+    assert L.noit_resolve(ctx._ctx, None, None) == 1
+    assert b"desc is NULL" in L.noit_last_error(ctx._ctx)
+    launches = ctx.launch_count
+    out = torch.full((fb.num_pixels, 4), 7.0, device="cuda")
+    d = ctx.make_resolve_desc(fb, BG, out_final=out)
+    d.full.width = 0
+    assert L.noit_resolve(ctx._ctx, C.byref(d), None) == 2
+    d = ctx.make_resolve_desc(fb, BG, out_final=out)
+    d.full.color_fmt = 9
+    assert L.noit_resolve(ctx._ctx, C.byref(d), None) == 3
+    d = ctx.make_resolve_desc(fb, BG, out_final=out)
+    d.out_final = out.data_ptr() + 4                             # misaligned
+    assert L.noit_resolve(ctx._ctx, C.byref(d), None) == 3
+    d = ctx.make_resolve_desc(fb, BG)
+    assert L.noit_resolve(ctx._ctx, C.byref(d), None) == 1       # every output NULL
+    torch.cuda.synchronize()
+    assert ctx.launch_count == launches and torch.all(out == 7.0)   # nothing ran, outputs untouched
+    with pytest.raises(noit.NoitError):
+        ctx.quadtree(out, 0, 64)
+    assert L.noit_infer(ctx._ctx, None, C.c_uint32(5), None, None) == 1
+    assert L.noit_last_error(None) is not None
