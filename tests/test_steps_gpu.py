@@ -24,16 +24,16 @@ def qt_equal(got, ref):
 @pytest.mark.parametrize("metric", [0, 1])
 def test_quadtree_random_images(noit, W, H, metric):
     rng = np.random.default_rng(W * 7 + H + metric)
-    # smooth field + blocks of noise so that every level of the tree occurs
+    # very smooth field + 16-px blocks of noise of three amplitudes, so that every level occurs
     yy, xx = np.mgrid[0:H, 0:W]
     img = np.zeros((H, W, 4), np.float32)
     for c in range(3):
-        img[..., c] = 0.5 + 0.3 * np.sin(xx / (40.0 + 10 * c)) * np.cos(yy / 55.0)
+        img[..., c] = 0.5 + 0.004 * np.sin(xx / (300.0 + 50 * c)) * np.cos(yy / 400.0)
     noise = rng.random((H, W, 3)).astype(np.float32)
-    sel = (rng.random((-(-H // 16), -(-W // 16))) < 0.3).repeat(16, 0).repeat(16, 1)[:H, :W]
-    amp = rng.choice([0.0, 0.02, 0.3], size=sel.shape).astype(np.float32)
+    sel = (rng.random((-(-H // 16), -(-W // 16))) < 0.12).repeat(16, 0).repeat(16, 1)[:H, :W]
+    amp = rng.choice([0.01, 0.05, 0.6], size=(-(-H // 16), -(-W // 16))).astype(np.float32)
+    amp = amp.repeat(16, 0).repeat(16, 1)[:H, :W]
     img[..., :3] += (sel * amp)[..., None] * (noise - 0.5)
-    img[..., :3] += (rng.random((H, W, 3)) < 0.001) * 2.0 - (rng.random((H, W, 3)) < 0.001) * 2.0
     img[..., 3] = rng.random((H, W))
     img = np.ascontiguousarray(img.reshape(-1, 4))
     ctx = noit.Noit()
@@ -42,8 +42,8 @@ def test_quadtree_random_images(noit, W, H, metric):
         ref = oracle.quadtree(img, W, H, metric, thr, cthr)
         qt_equal(got, ref)
     levels = set(np.unique(oracle.quadtree(img, W, H, metric, 6, 0.02)["cell_level"]).tolist())
-    if W >= 200:
-        assert levels == {0, 1, 2, 3} or metric == 1
+    if W >= 1920 and metric == 0:
+        assert levels == {0, 1, 2, 3}
 
 
 def test_quadtree_constant_image(noit):
