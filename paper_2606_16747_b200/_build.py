@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnoit.so")
-SOURCES = ["noit_api.cu", "noit_features.cu", "noit_resolve.cu", "noit_resolve_ring.cu",
+SOURCES = ["noit_api.cu", "noit_features.cu", "noit_resolve.cu", "noit_resolve_staged.cu",
            "noit_quadtree.cu", "noit_reproject.cu"]
 # no -use_fast_math anywhere: IEEE division / sqrt are part of the bit-exact classes
 COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -273,12 +273,15 @@ class Noit:
         import numpy as np
         P, dev = width * height, prev_trans.device
         out = dict(out) if out else {}
-        out.setdefault("trans", torch.zeros((P, 4), dtype=torch.float32, device=dev))
-        out.setdefault("depth", torch.zeros(P, dtype=torch.float32, device=dev))
-        out.setdefault("final", torch.zeros((P, 4), dtype=torch.float32, device=dev))
-        out.setdefault("accept", torch.empty(P, dtype=torch.uint8, device=dev))
-        out.setdefault("reject_list", torch.empty(P, dtype=torch.int32, device=dev))
-        out.setdefault("reject_count", torch.empty(1, dtype=torch.int32, device=dev))
+        mk = dict(trans=lambda: torch.zeros((P, 4), dtype=torch.float32, device=dev),
+                  depth=lambda: torch.zeros(P, dtype=torch.float32, device=dev),
+                  final=lambda: torch.zeros((P, 4), dtype=torch.float32, device=dev),
+                  accept=lambda: torch.empty(P, dtype=torch.uint8, device=dev),
+                  reject_list=lambda: torch.empty(P, dtype=torch.int32, device=dev),
+                  reject_count=lambda: torch.empty(1, dtype=torch.int32, device=dev))
+        for k, f in mk.items():          # allocate (and zero-fill) only what the caller did not pass
+            if k not in out:
+                out[k] = f()
         d = ReprojectDescC()
         d.width, d.height = width, height
         d.M = (C.c_float * 16)(*np.asarray(M, np.float32).reshape(-1).tolist())

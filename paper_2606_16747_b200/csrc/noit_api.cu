@@ -103,6 +103,19 @@ noit_status noit_set_weights(noit_ctx* ctx, const float* host_w, int32_t count, 
     float* dst = reinterpret_cast<float*>(&ctx->w);
     for (int i = 0; i < NOIT_MLP_PARAMS; ++i)
         dst[i] = precision == NOIT_MLP_BF16 ? round_bf16(host_w[i]) : host_w[i];
+    memset(&ctx->wt, 0, sizeof ctx->wt);
+    for (int o = 0; o < 32; ++o) {
+        for (int i = 0; i < 5; ++i) ctx->wt.w1t[i][o] = ctx->w.w1[o][i];
+        ctx->wt.b1[o] = ctx->w.b1[o];
+    }
+    for (int o = 0; o < 16; ++o) {
+        for (int i = 0; i < 32; ++i) ctx->wt.w2t[i][o] = ctx->w.w2[o][i];
+        ctx->wt.b2[o] = ctx->w.b2[o];
+    }
+    for (int o = 0; o < 3; ++o) {
+        for (int i = 0; i < 16; ++i) ctx->wt.w3t[i][o] = ctx->w.w3[o][i];
+        ctx->wt.b3[o] = ctx->w.b3[o];
+    }
     ctx->precision = precision;
     ctx->has_weights = true;
     return NOIT_OK;

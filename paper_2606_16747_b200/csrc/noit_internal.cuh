@@ -23,11 +23,24 @@ struct MlpWeights {
 };
 static_assert(sizeof(MlpWeights) == NOIT_MLP_PARAMS * 4, "771 parameters (P:97)");
 
+// The same parameters, input-major and padded, for the FFMA2 form of the MLP (two adjacent output
+// neurons per instruction): w1t[i][o], w2t[i][o], w3t[i][o] with o padded to 4 in layer 3.
+struct MlpWeightsT {
+    float w1t[5][32];
+    float b1[32];
+    float w2t[32][16];
+    float b2[16];
+    float w3t[16][4];
+    float b3[4];
+};
+static_assert(sizeof(MlpWeightsT) <= 4096, "fits the classic kernel-parameter space");
+
 struct noit_ctx {
     int device = 0;
     bool has_weights = false;
     int precision = 0;
     MlpWeights w;                    // effective weights, host copy (kernel argument source)
+    MlpWeightsT wt;                  // the same weights, input-major (FFMA2 form)
     void* d_mlp = nullptr;           // device copy of the packed tensor-core operands (bf16 path)
     uint64_t launches = 0;
     char err[512] = {0};
@@ -146,6 +159,56 @@ __device__ __forceinline__ void mlp_forward(const MlpWeights& W, const float x[5
         for (int i = 0; i < 16; ++i) a = fmaf(W.w3[o][i], h2[i], a);
         f[o] = fmaxf(a, 0.f);
     }
+}
+
+// fma.rn.f32x2 (sm_100): two independent IEEE fp32 FMAs in one instruction (SASS FFMA2).
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    unsigned long long ra = *reinterpret_cast<unsigned long long*>(&a);
+    unsigned long long rb = *reinterpret_cast<unsigned long long*>(&b);
+    unsigned long long rc = *reinterpret_cast<unsigned long long*>(&c);
+    unsigned long long rd;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    return *reinterpret_cast<float2*>(&rd);
+}
+
+// O4 with FFMA2: output neurons (o, o+1) share one instruction; each dot product still starts
+// from its bias and runs in input-index order, so the result is bit-identical to mlp_forward.
+__device__ __forceinline__ void mlp_forward_packed(const MlpWeightsT& W, const float x[5], float f[3])
+{
+    float2 h1[16], h2[8], h3[2];
+#pragma unroll
+    for (int o = 0; o < 16; ++o) h1[o] = make_float2(W.b1[2 * o], W.b1[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 5; ++i) {
+        const float2 xi = make_float2(x[i], x[i]);
+#pragma unroll
+        for (int o = 0; o < 16; ++o)
+            h1[o] = fma2(make_float2(W.w1t[i][2 * o], W.w1t[i][2 * o + 1]), xi, h1[o]);
+    }
+#pragma unroll
+    for (int o = 0; o < 8; ++o) h2[o] = make_float2(W.b2[2 * o], W.b2[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float v = fmaxf((i & 1) ? h1[i >> 1].y : h1[i >> 1].x, 0.f);
+        const float2 hi = make_float2(v, v);
+#pragma unroll
+        for (int o = 0; o < 8; ++o)
+            h2[o] = fma2(make_float2(W.w2t[i][2 * o], W.w2t[i][2 * o + 1]), hi, h2[o]);
+    }
+#pragma unroll
+    for (int o = 0; o < 2; ++o) h3[o] = make_float2(W.b3[2 * o], W.b3[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float v = fmaxf((i & 1) ? h2[i >> 1].y : h2[i >> 1].x, 0.f);
+        const float2 hi = make_float2(v, v);
+#pragma unroll
+        for (int o = 0; o < 2; ++o)
+            h3[o] = fma2(make_float2(W.w3t[i][2 * o], W.w3t[i][2 * o + 1]), hi, h3[o]);
+    }
+    f[0] = fmaxf(h3[0].x, 0.f);
+    f[1] = fmaxf(h3[0].y, 0.f);
+    f[2] = fmaxf(h3[1].x, 0.f);
 }
 
 // O3 features from raw accumulators; returns has_tail (A2).

@@ -1,11 +1,11 @@
 // noit_resolve.cu -- noit_resolve / noit_resolve_host: host-side checks and dispatch, plus the
 // GENERAL resolve kernel (one pixel per thread, fragments read straight from global memory).
-// The general kernel serves S9 (scattered pixel list), S7 (adaptive, per-tile LOD) and any
-// plain frame the staged ring kernel (noit_resolve_ring.cu) does not take.
+// The general kernel serves S9 (scattered pixel list) and S7 (adaptive, per-tile LOD); plain
+// frames go to the staged kernel (noit_resolve_staged.cu).
 #include "noit_resolve_common.cuh"
 
-noit_status noit_launch_resolve_ring(noit_ctx* ctx, const ResolveArgs& A, int color_fmt,
-                                     cudaStream_t st, bool* taken);
+noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt,
+                                       cudaStream_t st);
 
 enum { MODE_ALL = 0, MODE_LIST = 1, MODE_ADAPTIVE = 2 };
 
@@ -163,6 +163,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
     A.W = d->full.width;
     A.H = d->full.height;
     A.P = (uint32_t)A.W * (uint32_t)A.H;
+    A.F = d->full.num_fragments;
     A.offsets = d->full.offsets;
     A.depth = d->full.depth;
     A.rgba = d->full.rgba;
@@ -221,14 +222,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
         NOIT_CUDA(ctx, cudaGetLastError());
         return NOIT_OK;
     }
-    bool taken = false;                                    // plain frame: staged ring kernel
-    NOIT_TRY(noit_launch_resolve_ring(ctx, A, fmt, st, &taken));
-    if (!taken) {
-        launch_general<MODE_ALL>(A, ctx->w, fmt, (A.P + 127) / 128, st);
-        ctx->launches += 1;
-        NOIT_CUDA(ctx, cudaGetLastError());
-    }
-    return NOIT_OK;
+    return noit_launch_resolve_staged(ctx, A, fmt, st);     // plain frame: staged kernel
 }
 
 extern "C" {

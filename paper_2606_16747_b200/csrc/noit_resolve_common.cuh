@@ -4,7 +4,7 @@
 #include "noit_internal.cuh"
 
 struct ResolveArgs {
-    uint32_t P;
+    uint32_t P, F;
     int32_t W, H;
     const uint32_t* offsets;
     const float* depth;
@@ -21,9 +21,9 @@ struct ResolveArgs {
     uint8_t level_to_lod[4];
     const float* coarse_g[2];      // G[10] per coarse pixel, lod 1 (half) and lod 2 (quarter)
     int32_t coarse_w[2], coarse_h[2];
-    // ring kernel
+    // staged kernel
     uint32_t num_tiles;
-    uint32_t* tile_counter;
+    uint32_t* tile_counter;        // [0] next tile, [1] finished warps; self-resetting
 };
 
 #ifdef __CUDACC__

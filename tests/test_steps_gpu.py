@@ -97,10 +97,13 @@ def test_adaptive_resolve_small(noit, cfg4_small):
     for k in ("trans", "final"):
         close(got[k].cpu().numpy(), ref[k], extra=extra)
         assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
-    # all levels -> lod 0 is bitwise the plain resolve
+    # all levels -> lod 0 is the plain resolve (O7 pin).  The plain frame runs in the staged
+    # kernel (4 lanes per pixel), the adaptive frame in the one-thread-per-pixel kernel: same
+    # selection, different fp32 summation order => layer-1 depth bitwise, colours to tolerance.
     _, got0, _, _ = run_adaptive(noit, sc, l2l=(0, 0, 0, 0))
-    for k in ("trans", "final", "depth1"):
-        assert torch.equal(got0[k], plain[k]), k
+    assert torch.equal(got0["depth1"], plain["depth1"])
+    for k in ("trans", "final"):
+        close(got0[k].cpu().numpy(), plain[k].cpu().numpy().astype(np.float64), extra=extra)
 
 
 def test_adaptive_all_coarse(noit, cfg4_small):
@@ -174,7 +177,10 @@ def test_reproject_perspective_path(noit):
 
 def test_fallback_resolve_on_reject_list(noit):
     """S8 + S9: union of accepted and re-resolved pixels covers the frame exactly once; with a
-    negative threshold everything is rejected and the frame equals the plain resolve bitwise."""
+    negative threshold everything is rejected and the frame equals the plain resolve (layer-1
+    depth bitwise; colours to the fp32 tolerance, because the plain frame runs in the staged
+    kernel and the listed pixels in the one-thread-per-pixel kernel: same selection, different
+    fp32 summation order)."""
     rng = np.random.default_rng(23)
     W, H = 160, 96
     fbh = random_fb(rng, W, H, 24, np.float16)
@@ -198,12 +204,15 @@ def test_fallback_resolve_on_reject_list(noit):
         oracle.resolve(fbh, w_eff, BG, pixel_list=ref_rp["reject_list"], out=ref)
         for k in ("trans", "final"):
             assert np.max(np.abs(out[k].cpu().numpy() - ref[k])) <= 2e-3
-        for k in ("trans", "final", "depth1"):                                 # rejected == plain
-            assert torch.equal(out[k][~torch.from_numpy(acc).cuda()], plain[k][~torch.from_numpy(acc).cuda()])
+        rej = ~torch.from_numpy(acc).cuda()                                    # rejected == plain
+        lay = oracle.build_features(fbh)
+        mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+        extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)[~acc]
+        assert torch.equal(out["depth1"][rej], plain["depth1"][rej])
+        for k in ("trans", "final"):
+            close(out[k][rej].cpu().numpy(), plain[k][rej].cpu().numpy(), extra=extra)
         if thr < 0:
             assert n == W * H
-            for k in ("trans", "final", "depth1"):
-                assert torch.equal(out[k], plain[k])
 
 
 # -------------------------------------------------------------------------------------------
