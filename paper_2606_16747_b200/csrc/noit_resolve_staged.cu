@@ -1,6 +1,6 @@
 // noit_resolve_staged.cu -- the plain fused resolve (S1-S5, Eq. 4) of a whole frame:
 // persistent warps, fragment ranges staged into shared memory by 1-D TMA bulk copies
-// (cp.async.bulk + mbarrier), L lanes per pixel, MLP with packed FFMA2.
+// (cp.async.bulk + mbarrier), two passes over the staged lists, MLP with packed FFMA2.
 //
 // Why this shape (ncu evidence in profiles/r01_*): a thread-per-pixel kernel that reads its
 // list straight from global memory is bound by L1 data-stage wavefronts (every lane of a load
@@ -8,27 +8,32 @@
 // 48 % of the HBM roofline) and by its instruction count (36 per fragment, ~1000 per MLP).
 // Here
 //   * a WARP owns a tile of 32 consecutive pixels; their CSR lists are one contiguous fragment
-//     range, which lane 0 copies into the warp's private shared-memory stage with two bulk
-//     copies (depth, colour) that complete on the warp's mbarrier: no LSU wavefronts, no
-//     registers, fully coalesced HBM reads;
-//   * the tile is processed in L rounds of 32/L pixels with L lanes per pixel: lane q of a
-//     group reads fragments b+q, b+q+L, ... so a warp-wide shared-memory load reads 32/L runs of
-//     L consecutive words (few bank conflicts whatever the list lengths are, no alignment
-//     peeling), and the loop trip count is max over 32/L pixels of ceil(n/L);
+//     range, which lane 0 copies into the warp's private shared-memory stage with bulk copies
+//     that complete on the warp's mbarrier: no LSU wavefronts, no registers, coalesced HBM reads;
 //   * selection and reduction are two passes over the staged list: pass 1 tracks
-//     (d1,i1,d2,i2) on the depths only; the group merges its partial top-2 under the key
-//     (depth, index) (O1); the owner lane fetches the two layer colours and overwrites their
-//     alpha with 0 in the stage; pass 2 then accumulates EVERY staged fragment of the pixel
-//     (a zero alpha adds 0 and multiplies by 1), so the tail is never "all minus top-2" (O2);
-//   * after L rounds every lane owns one pixel: features, MLP (FFMA2: two output neurons per
+//     (d1,i1,d2,i2) on the depths only; the owner lane fetches the two layer colours and
+//     overwrites their alpha with 0 in the stage; pass 2 then accumulates EVERY staged fragment
+//     of the pixel (a zero alpha adds 0 and multiplies by 1), so the tail is never "all minus
+//     top-2" (O2) and pass 2 has no per-fragment test;
+//   * LIGHT tiles (all 32 lists fit the stage: 76 % of cfg3's tiles, 9 fragments per pixel on
+//     average) run one lane per pixel: no shuffles, no merges -- there the per-tile overhead,
+//     not the per-fragment work, is what counts;
+//   * HEAVY tiles (72 fragments per pixel on average in cfg3) run L = 4 lanes per pixel in 4
+//     rounds of 8 pixels (lane q of a group reads fragments b+q, b+q+4, ...: balanced trip
+//     counts, few bank conflicts).  The stage is used twice: first for depths only (3x the
+//     fragments fit), pass 1 of all rounds, ONE transposed butterfly that leaves lane q of a
+//     group with round q's merged top-2 (log2(L) exchange steps, L-1 merges, instead of L full
+//     butterflies); then for colours only, in chunks of rounds, pass 2, and one transposed
+//     butterfly of the five sums;
+//   * every lane then owns one pixel: features, MLP (FFMA2: two output neurons per
 //     instruction, same summation order as the scalar form), composite, 128-bit stores.
-// Tiles are handed out by an atomic counter (fragment counts vary 0..128 per pixel), which the
-// last warp to finish resets, so a launch needs no memset.
+// Tiles are handed out by an atomic counter (fragment counts vary 0..128 per pixel) whose result
+// is broadcast one tile later, and which the last warp to finish resets (no memset per launch).
 #include "noit_resolve_common.cuh"
 
 namespace {
 
-constexpr uint32_t kCap = 1032;          // fragments per warp stage: 8 px * 128 + alignment slack
+constexpr uint32_t kCap = 1032;          // fragments per warp stage: 8 px * 128 + alignment slack (16 warps/SM)
 constexpr int kWarpsPerCta = 4;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
@@ -105,18 +110,11 @@ __device__ __forceinline__ bool key_less(float da, uint32_t ia, float db, uint32
 
 }  // namespace
 
-// ------------------------------------------------------------------------------------------
-// the kernel
-// ------------------------------------------------------------------------------------------
-// One warp's private stage.
-template <typename ColorT>
-struct WarpStage {
-    float depth[kCap];
-    typename Color<ColorT>::Packed rgba[kCap];
-};
 
-// Per-lane results of the rounds: after round r the lanes with (lane % L) == r own pixel
-// r*(32/L) + lane/L of the tile.
+// ------------------------------------------------------------------------------------------
+// building blocks
+// ------------------------------------------------------------------------------------------
+// What a lane owns at the end of a tile.
 template <typename ColorT>
 struct Owned {
     typename Color<ColorT>::Packed c1, c2;
@@ -125,267 +123,183 @@ struct Owned {
     float acc_r, acc_g, acc_b, a_tail, t_tail;
 };
 
-// One round: pixels r*PPR .. r*PPR+PPR-1 of the tile, L lanes each.  D / C point at fragment
-// `base` (shared-memory stage when kStaged, global arrays with base = 0 otherwise).  Fragments
-// are addressed by their position relative to `base`; positions order like fragment indices.
-template <typename ColorT, int L, bool kStaged>
-__device__ __forceinline__ void resolve_round_body(int r, int lane, uint32_t o0, uint32_t o1,
-                                                   const float* D, typename Color<ColorT>::Packed* C,
-                                                   uint32_t base, Owned<ColorT>& own)
+struct Top2 { float d1, d2; uint32_t i1, i2; };
+struct Sums { float r, g, b, a, t; };
+
+// newcomer at a larger index wins a slot only on a strictly smaller depth (O1 tie rule)
+__device__ __forceinline__ void top2_push(Top2& s, float d, uint32_t pos)
+{
+    const bool lt1 = d < s.d1, lt2 = d < s.d2;
+    s.i2 = lt1 ? s.i1 : (lt2 ? pos : s.i2);
+    s.d2 = lt1 ? s.d1 : (lt2 ? d : s.d2);
+    s.i1 = lt1 ? pos : s.i1;
+    s.d1 = lt1 ? d : s.d1;
+}
+// merge another sorted pair into s under the key (depth, index)
+__device__ __forceinline__ void top2_merge(Top2& s, float od1, uint32_t oi1, float od2, uint32_t oi2)
+{
+    const bool mine = key_less(s.d1, s.i1, od1, oi1);
+    const float xd = mine ? s.d2 : od2, yd = mine ? od1 : s.d1;     // runner-up of the winner side,
+    const uint32_t xi = mine ? s.i2 : oi2, yi = mine ? oi1 : s.i1;  // best of the loser side
+    const bool xy = key_less(xd, xi, yd, yi);
+    s.d1 = mine ? s.d1 : od1;
+    s.i1 = mine ? s.i1 : oi1;
+    s.d2 = xy ? xd : yd;
+    s.i2 = xy ? xi : yi;
+}
+
+// pass 1 over positions first, first+S, ... < end of the staged depths
+template <int S>
+__device__ __forceinline__ Top2 scan_depths(const float* D, uint32_t first, uint32_t end)
+{
+    Top2 s;
+    s.d1 = s.d2 = __int_as_float(0x7f800000);
+    s.i1 = s.i2 = NOIT_ABSENT;
+    uint32_t pos = first;
+#pragma unroll 1
+    for (; pos + S < end; pos += 2 * S) {
+        const float da = D[pos], db = D[pos + S];
+        top2_push(s, da, pos);
+        top2_push(s, db, pos + S);
+    }
+    if (pos < end) top2_push(s, D[pos], pos);
+    return s;
+}
+// pass 2 over the same positions of the staged colours (layers carry alpha 0)
+template <typename ColorT, int S>
+__device__ __forceinline__ Sums scan_colours(const typename Color<ColorT>::Packed* C, uint32_t first,
+                                             uint32_t end)
 {
     typedef typename Color<ColorT>::Packed Packed;
-    constexpr int PPR = 32 / L;
-    const int g = lane / L, q = lane % L;
-    const int px = r * PPR + g;
-    const uint32_t b = __shfl_sync(0xffffffffu, o0, px), e = __shfl_sync(0xffffffffu, o1, px);
-    const uint32_t first = b - base + q, end = e - base;
-
-    // ---- pass 1: partial top-2 over this lane's fragments, in increasing index order, so a
-    // newcomer wins a slot only on a strictly smaller depth (ties keep the earlier index, O1)
-    float d1 = __int_as_float(0x7f800000), d2 = d1;
-    uint32_t i1 = NOIT_ABSENT, i2 = NOIT_ABSENT;
-    auto step1 = [&](float d, uint32_t pos) {
-        const bool lt1 = d < d1, lt2 = d < d2;
-        i2 = lt1 ? i1 : (lt2 ? pos : i2);
-        d2 = lt1 ? d1 : (lt2 ? d : d2);
-        i1 = lt1 ? pos : i1;
-        d1 = lt1 ? d : d1;
-    };
-    {
-        uint32_t pos = first;
-#pragma unroll 1
-        for (; pos + L < end; pos += 2 * L) {
-            const float da = D[pos], db = D[pos + L];
-            step1(da, pos);
-            step1(db, pos + L);
-        }
-        if (pos < end) step1(D[pos], pos);
-    }
-    // ---- merge the L partial results (butterfly: every lane of the group ends with the result)
-#pragma unroll
-    for (int s = 1; s < L; s <<= 1) {
-        const float od1 = __shfl_xor_sync(0xffffffffu, d1, s), od2 = __shfl_xor_sync(0xffffffffu, d2, s);
-        const uint32_t oi1 = __shfl_xor_sync(0xffffffffu, i1, s), oi2 = __shfl_xor_sync(0xffffffffu, i2, s);
-        const bool mine = key_less(d1, i1, od1, oi1);
-        // x = runner-up of the winning side, y = best of the losing side
-        const float xd = mine ? d2 : od2, yd = mine ? od1 : d1;
-        const uint32_t xi = mine ? i2 : oi2, yi = mine ? oi1 : i1;
-        d1 = mine ? d1 : od1;
-        i1 = mine ? i1 : oi1;
-        const bool xy = key_less(xd, xi, yd, yi);
-        d2 = xy ? xd : yd;
-        i2 = xy ? xi : yi;
-    }
-    // ---- the owner lane fetches the two layers; their alpha is then neutralised for pass 2
-    const bool owner = q == r;
-    Packed c1 = Color<ColorT>::zero(), c2 = Color<ColorT>::zero();
-    if (owner) {
-        if (i1 != NOIT_ABSENT) {
-            c1 = C[i1];
-            if (kStaged) Color<ColorT>::zero_alpha(&C[i1]);
-        }
-        if (i2 != NOIT_ABSENT) {
-            c2 = C[i2];
-            if (kStaged) Color<ColorT>::zero_alpha(&C[i2]);
-        }
-    }
-    if (kStaged) __syncwarp();
-    // ---- pass 2: tail accumulators over every fragment of the pixel (layers carry alpha 0)
-    float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f;
-    auto step2 = [&](Packed raw, uint32_t pos) {
-        if (!kStaged && (pos == i1 || pos == i2)) raw = Color<ColorT>::zero_alpha_reg(raw);
+    Sums s;
+    s.r = s.g = s.b = s.a = 0.f;
+    s.t = 1.f;
+    auto acc = [&](Packed raw) {
         const float4 c = Color<ColorT>::unpack(raw);
-        ar = fmaf(c.w, c.x, ar);
-        ag = fmaf(c.w, c.y, ag);
-        ab = fmaf(c.w, c.z, ab);
-        at += c.w;
-        tt = fmaf(-c.w, tt, tt);                       // tt *= (1 - alpha), one rounding
+        s.r = fmaf(c.w, c.x, s.r);
+        s.g = fmaf(c.w, c.y, s.g);
+        s.b = fmaf(c.w, c.z, s.b);
+        s.a += c.w;
+        s.t = fmaf(-c.w, s.t, s.t);                    // t *= (1 - alpha), one rounding
     };
-    {
-        uint32_t pos = first;
+    uint32_t pos = first;
 #pragma unroll 1
-        for (; pos + L < end; pos += 2 * L) {
-            const Packed ra = C[pos], rb = C[pos + L];
-            step2(ra, pos);
-            step2(rb, pos + L);
-        }
-        if (pos < end) step2(C[pos], pos);
+    for (; pos + S < end; pos += 2 * S) {
+        const Packed ra = C[pos], rb = C[pos + S];
+        acc(ra);
+        acc(rb);
     }
-#pragma unroll
-    for (int s = 1; s < L; s <<= 1) {
-        ar += __shfl_xor_sync(0xffffffffu, ar, s);
-        ag += __shfl_xor_sync(0xffffffffu, ag, s);
-        ab += __shfl_xor_sync(0xffffffffu, ab, s);
-        at += __shfl_xor_sync(0xffffffffu, at, s);
-        tt *= __shfl_xor_sync(0xffffffffu, tt, s);
-    }
-    if (owner) {
-        own.c1 = c1; own.c2 = c2;
-        own.d1 = d1;
-        own.n = e - b;
-        own.acc_r = ar; own.acc_g = ag; own.acc_b = ab; own.a_tail = at; own.t_tail = tt;
-    }
+    if (pos < end) acc(C[pos]);
+    return s;
 }
 
-template <typename ColorT, int L>
-__device__ __forceinline__ void resolve_round_staged(int r, int lane, uint32_t o0, uint32_t o1,
-                                                     WarpStage<ColorT>* stage, uint32_t base,
-                                                     Owned<ColorT>& own)
+// Transposed butterfly over L items held by each of the L lanes of a group: at step m the
+// live slots are [0, 2m); a lane with bit m of q clear keeps slot r and sends slot r+m (r < m),
+// its partner q^m does the opposite; the combined item goes to slot r.  After the last step
+// slot 0 of lane q holds item q combined over the whole group.
+template <int L>
+__device__ __forceinline__ void transposed_merge(Top2 (&s)[L], int q)
 {
-    resolve_round_body<ColorT, L, true>(r, lane, o0, o1, stage->depth, stage->rgba, base, own);
-}
-// cold path: a round whose fragments do not fit the stage reads global memory directly
-template <typename ColorT, int L>
-__device__ __noinline__ Owned<ColorT> resolve_round_global(int r, int lane, uint32_t o0, uint32_t o1,
-                                                           const float* depth,
-                                                           typename Color<ColorT>::Packed* rgba,
-                                                           Owned<ColorT> own)
-{
-    resolve_round_body<ColorT, L, false>(r, lane, o0, o1, depth, rgba, 0u, own);
-    return own;
-}
-
-// A whole tile whose fragments are staged at once (the common case): pass 1 of all L rounds,
-// ONE transposed butterfly that leaves lane q of each group with the merged top-2 of the
-// group's round-q pixel (log2(L) exchange steps that halve the items a lane holds, instead of
-// L full butterflies), layer fetch + alpha neutralisation, one __syncwarp, pass 2 of all L
-// rounds, one transposed butterfly of the five sums.  Lane (g, q) ends up owning pixel
-// q*(32/L) + g.
-template <typename ColorT, int L>
-__device__ __forceinline__ void resolve_tile_staged(int lane, uint32_t o0, uint32_t o1,
-                                                    WarpStage<ColorT>* stage, uint32_t base,
-                                                    Owned<ColorT>& own)
-{
-    typedef typename Color<ColorT>::Packed Packed;
-    constexpr int PPR = 32 / L;
-    const int g = lane / L, q = lane % L;
-    const float* D = stage->depth;
-    Packed* C = stage->rgba;
-    float d1[L], d2[L];
-    uint32_t i1[L], i2[L], first[L], end[L];
-#pragma unroll
-    for (int r = 0; r < L; ++r) {
-        const int px = r * PPR + g;
-        const uint32_t b = __shfl_sync(0xffffffffu, o0, px), e = __shfl_sync(0xffffffffu, o1, px);
-        first[r] = b - base + q;
-        end[r] = e - base;
-        float a1 = __int_as_float(0x7f800000), a2 = a1;
-        uint32_t j1 = NOIT_ABSENT, j2 = NOIT_ABSENT;
-        auto step1 = [&](float d, uint32_t pos) {
-            const bool lt1 = d < a1, lt2 = d < a2;
-            j2 = lt1 ? j1 : (lt2 ? pos : j2);
-            a2 = lt1 ? a1 : (lt2 ? d : a2);
-            j1 = lt1 ? pos : j1;
-            a1 = lt1 ? d : a1;
-        };
-        uint32_t pos = first[r];
-#pragma unroll 1
-        for (; pos + L < end[r]; pos += 2 * L) {
-            const float da = D[pos], db = D[pos + L];
-            step1(da, pos);
-            step1(db, pos + L);
-        }
-        if (pos < end[r]) step1(D[pos], pos);
-        d1[r] = a1; d2[r] = a2; i1[r] = j1; i2[r] = j2;
-    }
-    // transposed butterfly: at step m the live slots are [0, 2m); a lane with bit m of q clear
-    // keeps slot r and sends slot r + m (r < m), its partner q ^ m does the opposite; both
-    // slots hold the same two items on both lanes, the merged item goes to slot r.  After the
-    // last step slot 0 holds item (round) q.
-#pragma unroll
-    for (int m = L / 2; m >= 1; m >>= 1) {
-        const bool up = (q & m) != 0;
-#pragma unroll
-        for (int r = 0; r < L; ++r) {
-            if (r >= m) continue;       // live slots are [0, 2m): pair slot r with slot r + m
-            const int rk0 = r, rk1 = r + m;
-            // keep = up ? item[rk1] : item[rk0];  send = up ? item[rk0] : item[rk1]
-            const float kd1 = up ? d1[rk1] : d1[rk0], kd2 = up ? d2[rk1] : d2[rk0];
-            const uint32_t ki1 = up ? i1[rk1] : i1[rk0], ki2 = up ? i2[rk1] : i2[rk0];
-            const float sd1 = up ? d1[rk0] : d1[rk1], sd2 = up ? d2[rk0] : d2[rk1];
-            const uint32_t si1 = up ? i1[rk0] : i1[rk1], si2 = up ? i2[rk0] : i2[rk1];
-            const float od1 = __shfl_xor_sync(0xffffffffu, sd1, m), od2 = __shfl_xor_sync(0xffffffffu, sd2, m);
-            const uint32_t oi1 = __shfl_xor_sync(0xffffffffu, si1, m), oi2 = __shfl_xor_sync(0xffffffffu, si2, m);
-            const bool mine = key_less(kd1, ki1, od1, oi1);
-            const float xd = mine ? kd2 : od2, yd = mine ? od1 : kd1;
-            const uint32_t xi = mine ? ki2 : oi2, yi = mine ? oi1 : ki1;
-            const bool xy = key_less(xd, xi, yd, yi);
-            // the merged item is stored in slot rk0 (slot index with bit m cleared)
-            d1[rk0] = mine ? kd1 : od1;
-            i1[rk0] = mine ? ki1 : oi1;
-            d2[rk0] = xy ? xd : yd;
-            i2[rk0] = xy ? xi : yi;
-        }
-    }
-    // slot 0 now holds the merged top-2 of pixel q*PPR + g
-    Packed c1 = Color<ColorT>::zero(), c2 = Color<ColorT>::zero();
-    if (i1[0] != NOIT_ABSENT) {
-        c1 = C[i1[0]];
-        Color<ColorT>::zero_alpha(&C[i1[0]]);
-    }
-    if (i2[0] != NOIT_ABSENT) {
-        c2 = C[i2[0]];
-        Color<ColorT>::zero_alpha(&C[i2[0]]);
-    }
-    __syncwarp();
-    float ar[L], ag[L], ab[L], at[L], tt[L];
-#pragma unroll
-    for (int r = 0; r < L; ++r) {
-        float xr = 0.f, xg = 0.f, xb = 0.f, xa = 0.f, xt = 1.f;
-        auto step2 = [&](Packed raw) {
-            const float4 c = Color<ColorT>::unpack(raw);
-            xr = fmaf(c.w, c.x, xr);
-            xg = fmaf(c.w, c.y, xg);
-            xb = fmaf(c.w, c.z, xb);
-            xa += c.w;
-            xt = fmaf(-c.w, xt, xt);                   // xt *= (1 - alpha), one rounding
-        };
-        uint32_t pos = first[r];
-#pragma unroll 1
-        for (; pos + L < end[r]; pos += 2 * L) {
-            const Packed ra = C[pos], rb = C[pos + L];
-            step2(ra);
-            step2(rb);
-        }
-        if (pos < end[r]) step2(C[pos]);
-        ar[r] = xr; ag[r] = xg; ab[r] = xb; at[r] = xa; tt[r] = xt;
-    }
 #pragma unroll
     for (int m = L / 2; m >= 1; m >>= 1) {
         const bool up = (q & m) != 0;
 #pragma unroll
         for (int r = 0; r < L; ++r) {
             if (r >= m) continue;
-            const int rk0 = r, rk1 = r + m;
-            const float sr = up ? ar[rk0] : ar[rk1], sg = up ? ag[rk0] : ag[rk1];
-            const float sb = up ? ab[rk0] : ab[rk1], sa = up ? at[rk0] : at[rk1];
-            const float st = up ? tt[rk0] : tt[rk1];
-            ar[rk0] = (up ? ar[rk1] : ar[rk0]) + __shfl_xor_sync(0xffffffffu, sr, m);
-            ag[rk0] = (up ? ag[rk1] : ag[rk0]) + __shfl_xor_sync(0xffffffffu, sg, m);
-            ab[rk0] = (up ? ab[rk1] : ab[rk0]) + __shfl_xor_sync(0xffffffffu, sb, m);
-            at[rk0] = (up ? at[rk1] : at[rk0]) + __shfl_xor_sync(0xffffffffu, sa, m);
-            tt[rk0] = (up ? tt[rk1] : tt[rk0]) * __shfl_xor_sync(0xffffffffu, st, m);
+            Top2 keep = up ? s[r + m] : s[r];
+            const Top2 send = up ? s[r] : s[r + m];
+            top2_merge(keep, __shfl_xor_sync(0xffffffffu, send.d1, m), __shfl_xor_sync(0xffffffffu, send.i1, m),
+                       __shfl_xor_sync(0xffffffffu, send.d2, m), __shfl_xor_sync(0xffffffffu, send.i2, m));
+            s[r] = keep;
         }
     }
-    own.c1 = c1; own.c2 = c2;
-    own.d1 = d1[0];
-    own.n = __shfl_sync(0xffffffffu, o1 - o0, q * PPR + g);
-    own.acc_r = ar[0]; own.acc_g = ag[0]; own.acc_b = ab[0]; own.a_tail = at[0]; own.t_tail = tt[0];
+}
+template <int L>
+__device__ __forceinline__ void transposed_sum(Sums (&s)[L], int q)
+{
+#pragma unroll
+    for (int m = L / 2; m >= 1; m >>= 1) {
+        const bool up = (q & m) != 0;
+#pragma unroll
+        for (int r = 0; r < L; ++r) {
+            if (r >= m) continue;
+            const Sums keep = up ? s[r + m] : s[r];
+            const Sums send = up ? s[r] : s[r + m];
+            s[r].r = keep.r + __shfl_xor_sync(0xffffffffu, send.r, m);
+            s[r].g = keep.g + __shfl_xor_sync(0xffffffffu, send.g, m);
+            s[r].b = keep.b + __shfl_xor_sync(0xffffffffu, send.b, m);
+            s[r].a = keep.a + __shfl_xor_sync(0xffffffffu, send.a, m);
+            s[r].t = keep.t * __shfl_xor_sync(0xffffffffu, send.t, m);
+        }
+    }
 }
 
+// ---- cold path: a tile with a round too long for the stage (lists far beyond BASELINE.json's
+// 128-fragment cap) reads global memory directly; the two layers are skipped by index in pass 2.
+template <typename ColorT, int L>
+__device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, uint32_t o1,
+                                                       const float* __restrict__ depth,
+                                                       const typename Color<ColorT>::Packed* __restrict__ rgba)
+{
+    constexpr int PPR = 32 / L;
+    const int g = lane / L, q = lane % L;
+    Owned<ColorT> own;
+    for (int r = 0; r < L; ++r) {
+        const int px = r * PPR + g;
+        const uint32_t b = __shfl_sync(0xffffffffu, o0, px), e = __shfl_sync(0xffffffffu, o1, px);
+        Top2 s;
+        s.d1 = s.d2 = __int_as_float(0x7f800000);
+        s.i1 = s.i2 = NOIT_ABSENT;
+        for (uint32_t j = b + q; j < e; j += L) top2_push(s, __ldg(depth + j), j);
+#pragma unroll
+        for (int m = 1; m < L; m <<= 1)
+            top2_merge(s, __shfl_xor_sync(0xffffffffu, s.d1, m), __shfl_xor_sync(0xffffffffu, s.i1, m),
+                       __shfl_xor_sync(0xffffffffu, s.d2, m), __shfl_xor_sync(0xffffffffu, s.i2, m));
+        float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f;
+        for (uint32_t j = b + q; j < e; j += L) {
+            if (j == s.i1 || j == s.i2) continue;
+            const float4 c = Color<ColorT>::unpack(__ldg(rgba + j));
+            ar = fmaf(c.w, c.x, ar); ag = fmaf(c.w, c.y, ag); ab = fmaf(c.w, c.z, ab);
+            at += c.w;
+            tt = fmaf(-c.w, tt, tt);
+        }
+#pragma unroll
+        for (int m = 1; m < L; m <<= 1) {
+            ar += __shfl_xor_sync(0xffffffffu, ar, m); ag += __shfl_xor_sync(0xffffffffu, ag, m);
+            ab += __shfl_xor_sync(0xffffffffu, ab, m); at += __shfl_xor_sync(0xffffffffu, at, m);
+            tt *= __shfl_xor_sync(0xffffffffu, tt, m);
+        }
+        if (q == r) {
+            own.c1 = s.i1 != NOIT_ABSENT ? __ldg(rgba + s.i1) : Color<ColorT>::zero();
+            own.c2 = s.i2 != NOIT_ABSENT ? __ldg(rgba + s.i2) : Color<ColorT>::zero();
+            own.d1 = s.d1;
+            own.n = e - b;
+            own.acc_r = ar; own.acc_g = ag; own.acc_b = ab; own.a_tail = at; own.t_tail = tt;
+        }
+    }
+    return own;
+}
+
+// ------------------------------------------------------------------------------------------
+// the kernel
+// ------------------------------------------------------------------------------------------
 template <typename ColorT, int L>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
 {
     typedef typename Color<ColorT>::Packed Packed;
     constexpr uint32_t CB = Color<ColorT>::kBytes;
+    constexpr uint32_t kStageBytes = kCap * (4u + CB);   // per warp
+    constexpr uint32_t kCapD = kStageBytes / 4u;         // fragments when the stage holds depths only
+    constexpr uint32_t kCapC = kStageBytes / CB;         // ... colours only
     constexpr int PPR = 32 / L;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpStage<ColorT>* stage = reinterpret_cast<WarpStage<ColorT>*>(smem_raw) + warp;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * sizeof(WarpStage<ColorT>));
-    const uint32_t bar = smem_u32(bars + warp);
-    const uint32_t s_depth = smem_u32(stage->depth), s_rgba = smem_u32(stage->rgba);
+    unsigned char* stage = smem_raw + warp * kStageBytes;
+    float* const sD = reinterpret_cast<float*>(stage);                   // depths (both views)
+    Packed* const sC2 = reinterpret_cast<Packed*>(stage + kCap * 4u);    // colours behind kCap depths
+    Packed* const sC = reinterpret_cast<Packed*>(stage);                 // colours only
+    const uint32_t bar = smem_u32(reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * kStageBytes) + warp);
     if (lane == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -396,26 +310,33 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     const uint32_t* __restrict__ offsets = A.offsets;
     const Packed* __restrict__ g_rgba = static_cast<const Packed*>(A.rgba);
 
-    auto fetch_tile = [&]() -> uint32_t {
+    // lane 0's atomic result is broadcast one tile later: its latency hides behind a tile
+    auto fetch_raw = [&]() -> uint32_t {
         uint32_t t = 0;
         if (lane == 0) t = atomicAdd(A.tile_counter, 1u);
-        return __shfl_sync(0xffffffffu, t, 0);
+        return t;
     };
-    // stage fragments [fs, fe) (fs a multiple of 4) into the warp's stage and wait for them
-    auto stage_range = [&](uint32_t fs, uint32_t fe) {
-        __syncwarp();                                   // everyone is done with the old contents
+    auto load_offsets = [&](uint32_t tile, uint32_t& a, uint32_t& b) {
+        const uint32_t p = tile * 32u + lane;
+        a = __ldg(offsets + min(p, A.P));
+        b = __ldg(offsets + min(p + 1u, A.P));
+    };
+    // Stage fragments [fs, fe) (fs a multiple of 4 = 16 bytes) and wait for them.  The bulk
+    // copies never read past the arrays: the last < 4 fragments of the frame are copied by lanes.
+    auto stage_range = [&](float* dst_d, Packed* dst_c, uint32_t fs, uint32_t fe) {
+        __syncwarp();                                   // nobody still reads the old contents
         uint32_t n4 = (fe - fs + 3u) & ~3u;
-        if (fs + n4 > A.F) n4 = (A.F - fs) & ~3u;       // never read past the arrays
+        if (fs + n4 > A.F) n4 = (A.F - fs) & ~3u;
         if (lane == 0 && n4) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_expect_tx(bar, n4 * (4u + CB));
-            bulk_g2s(s_depth, A.depth + fs, n4 * 4u, bar);
-            bulk_g2s(s_rgba, g_rgba + fs, n4 * CB, bar);
+            mbar_expect_tx(bar, n4 * ((dst_d ? 4u : 0u) + (dst_c ? CB : 0u)));
+            if (dst_d) bulk_g2s(smem_u32(dst_d), A.depth + fs, n4 * 4u, bar);
+            if (dst_c) bulk_g2s(smem_u32(dst_c), g_rgba + fs, n4 * CB, bar);
         }
-        const uint32_t rem = fe - fs > n4 ? fe - fs - n4 : 0u;   // < 4, last fragments of the frame
+        const uint32_t rem = fe - fs > n4 ? fe - fs - n4 : 0u;
         if ((uint32_t)lane < rem) {
-            stage->depth[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
-            stage->rgba[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
+            if (dst_d) dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
+            if (dst_c) dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
         }
         if (n4) {
             mbar_wait(bar, parity);
@@ -423,50 +344,119 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         }
         __syncwarp();
     };
-    auto load_offsets = [&](uint32_t tile, uint32_t& o0, uint32_t& o1) {
-        const uint32_t p = tile * 32u + lane;
-        o0 = __ldg(offsets + min(p, A.P));
-        o1 = __ldg(offsets + min(p + 1u, A.P));
-    };
 
-    uint32_t tile = fetch_tile(), o0 = 0, o1 = 0;
-    if (tile < A.num_tiles) load_offsets(tile, o0, o1);
-    while (tile < A.num_tiles) {
-        // next tile's index and offsets travel while this tile is processed
-        const uint32_t next = fetch_tile();
+    uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0);
+    uint32_t raw_nxt = fetch_raw();
+    uint32_t o0 = 0, o1 = 0;
+    if (t_cur < A.num_tiles) load_offsets(t_cur, o0, o1);
+    while (t_cur < A.num_tiles) {
+        const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
+        raw_nxt = fetch_raw();
         uint32_t no0 = 0, no1 = 0;
-        if (next < A.num_tiles) load_offsets(next, no0, no1);
+        if (t_nxt < A.num_tiles) load_offsets(t_nxt, no0, no1);   // lands while this tile runs
 
         Owned<ColorT> own;
         own.c1 = own.c2 = Color<ColorT>::zero();
         own.d1 = 1.0f; own.n = 0;
         own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
+        uint32_t px_own = lane;                          // pixel of the tile this lane ends up owning
 
         const uint32_t tb = __shfl_sync(0xffffffffu, o0, 0), te = __shfl_sync(0xffffffffu, o1, 31);
         const uint32_t fs = tb & ~3u;
-        const bool heavy = te - fs > kCap;               // warp-uniform
-        if (!heavy) {
+        if (te - fs <= kCap) {
+            // ---- light tile: one lane per pixel, depths and colours staged together
             if (te > tb) {
-                stage_range(fs, te);
-                resolve_tile_staged<ColorT, L>(lane, o0, o1, stage, fs, own);
+                stage_range(sD, sC2, fs, te);
+                const uint32_t first = o0 - fs, end = o1 - fs;
+                const Top2 s = scan_depths<1>(sD, first, end);
+                if (s.i1 != NOIT_ABSENT) {
+                    own.c1 = sC2[s.i1];
+                    Color<ColorT>::zero_alpha(&sC2[s.i1]);
+                }
+                if (s.i2 != NOIT_ABSENT) {
+                    own.c2 = sC2[s.i2];
+                    Color<ColorT>::zero_alpha(&sC2[s.i2]);
+                }
+                const Sums z = scan_colours<ColorT, 1>(sC2, first, end);    // own list only: no sync
+                own.d1 = s.d1;
+                own.n = o1 - o0;
+                own.acc_r = z.r; own.acc_g = z.g; own.acc_b = z.b; own.a_tail = z.a; own.t_tail = z.t;
             }
         } else {
-#pragma unroll 1
-            for (int r = 0; r < L; ++r) {                // stage round by round
-                const uint32_t rb = __shfl_sync(0xffffffffu, o0, r * PPR);
-                const uint32_t re = __shfl_sync(0xffffffffu, o1, r * PPR + PPR - 1);
-                const uint32_t base = rb & ~3u;
-                if (re - base > kCap) {                  // lists longer than the stage
-                    own = resolve_round_global<ColorT, L>(r, lane, o0, o1, A.depth,
-                                                          const_cast<Packed*>(g_rgba), own);
-                    continue;
+            // ---- heavy tile: L lanes per pixel, L rounds of PPR pixels
+            const int g = lane / L, q = lane % L;
+            px_own = (uint32_t)(q * PPR + g);
+            uint32_t B[L + 1];                           // fragment bounds of the rounds
+#pragma unroll
+            for (int r = 0; r < L; ++r) B[r] = __shfl_sync(0xffffffffu, o0, r * PPR);
+            B[L] = te;
+            bool fits = true;
+#pragma unroll
+            for (int r = 0; r < L; ++r) fits = fits && (B[r + 1] - (B[r] & ~3u) <= kCapC);
+            if (!fits) {
+                own = tile_from_global<ColorT, L>(lane, o0, o1, A.depth, g_rgba);
+            } else {
+                Top2 t2[L];
+                uint32_t first[L], end[L];
+                int staged_to = 0;
+                const float* Dv = sD;                    // staged depths, indexed by fragment index
+#pragma unroll
+                for (int r = 0; r < L; ++r) {
+                    if (r == staged_to) {                // stage the next chunk of rounds (depths)
+                        int k = r + 1;
+                        uint32_t bk = B[r + 1];
+#pragma unroll
+                        for (int c = r + 1; c < L; ++c)
+                            if (k == c && B[c + 1] - (B[r] & ~3u) <= kCapD) { k = c + 1; bk = B[c + 1]; }
+                        const uint32_t base = B[r] & ~3u;
+                        if (bk > B[r]) stage_range(sD, nullptr, base, bk);
+                        Dv = sD - base;
+                        staged_to = k;
+                    }
+                    const int px = r * PPR + g;
+                    first[r] = __shfl_sync(0xffffffffu, o0, px) + q;
+                    end[r] = __shfl_sync(0xffffffffu, o1, px);
+                    t2[r] = scan_depths<L>(Dv, first[r], end[r]);
                 }
-                if (re > rb) stage_range(base, re);
-                resolve_round_staged<ColorT, L>(r, lane, o0, o1, stage, base, own);
+                transposed_merge<L>(t2, q);              // t2[0]: this lane's pixel, global indices
+                Sums sm[L];
+                staged_to = 0;
+                Packed* Cv = sC;
+#pragma unroll
+                for (int r = 0; r < L; ++r) {
+                    if (r == staged_to) {                // stage the next chunk of rounds (colours)
+                        int k = r + 1;
+                        uint32_t bk = B[r + 1];
+#pragma unroll
+                        for (int c = r + 1; c < L; ++c)
+                            if (k == c && B[c + 1] - (B[r] & ~3u) <= kCapC) { k = c + 1; bk = B[c + 1]; }
+                        const uint32_t base = B[r] & ~3u;
+                        if (bk > B[r]) stage_range(nullptr, sC, base, bk);
+                        Cv = sC - base;
+                        if (q >= r && q < k) {           // owners of the chunk's rounds
+                            if (t2[0].i1 != NOIT_ABSENT) {
+                                own.c1 = Cv[t2[0].i1];
+                                Color<ColorT>::zero_alpha(&Cv[t2[0].i1]);
+                            }
+                            if (t2[0].i2 != NOIT_ABSENT) {
+                                own.c2 = Cv[t2[0].i2];
+                                Color<ColorT>::zero_alpha(&Cv[t2[0].i2]);
+                            }
+                        }
+                        __syncwarp();
+                        staged_to = k;
+                    }
+                    sm[r] = scan_colours<ColorT, L>(Cv, first[r], end[r]);
+                }
+                transposed_sum<L>(sm, q);
+                own.d1 = t2[0].d1;
+                own.n = __shfl_sync(0xffffffffu, o1 - o0, (int)px_own);
+                own.acc_r = sm[0].r; own.acc_g = sm[0].g; own.acc_b = sm[0].b;
+                own.a_tail = sm[0].a; own.t_tail = sm[0].t;
             }
         }
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
-        const uint32_t p = tile * 32u + (uint32_t)((lane % L) * PPR + lane / L);
+        const uint32_t p = t_cur * 32u + px_own;
         if (p < A.P) {
             float xf[5], f[3];
             // O3 with one IEEE reciprocal instead of three divisions
@@ -479,7 +469,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             composite_store(A, p, c1, make_float4(c2.w * c2.x, c2.w * c2.y, c2.w * c2.z, c2.w),
                             own.n ? own.d1 : 1.0f, has_tail, f, own.t_tail);
         }
-        tile = next; o0 = no0; o1 = no1;
+        t_cur = t_nxt; o0 = no0; o1 = no1;
     }
     // the last warp to finish re-arms the counters for the next launch
     if (lane == 0) {
@@ -495,7 +485,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 template <typename ColorT, int L>
 static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
 {
-    const size_t smem = kWarpsPerCta * sizeof(WarpStage<ColorT>) + kWarpsPerCta * sizeof(uint64_t);
+    const size_t smem = kWarpsPerCta * (size_t)kCap * (4u + Color<ColorT>::kBytes) +
+                        kWarpsPerCta * sizeof(uint64_t);
     static bool configured = false;                     // per instantiation
     if (!configured) {
         NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L>,
