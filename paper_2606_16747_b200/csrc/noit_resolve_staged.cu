@@ -321,10 +321,12 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         a = __ldg(offsets + min(p, A.P));
         b = __ldg(offsets + min(p + 1u, A.P));
     };
-    // Stage fragments [fs, fe) (fs a multiple of 4 = 16 bytes) and wait for them.  The bulk
-    // copies never read past the arrays: the last < 4 fragments of the frame are copied by lanes.
-    auto stage_range = [&](float* dst_d, Packed* dst_c, uint32_t fs, uint32_t fe) {
-        __syncwarp();                                   // nobody still reads the old contents
+    // Issue the copy of fragments [fs, fe) (fs a multiple of 4 = 16 bytes) into the stage; the
+    // caller has made sure nobody still reads the old contents.  The bulk copies never read
+    // past the arrays: the last < 4 fragments of the frame are copied by lanes.
+    bool pend = false;                                   // warp-uniform: a bulk copy is in flight
+    auto issue_fill = [&](float* dst_d, Packed* dst_c, uint32_t fs, uint32_t fe) {
+        __syncwarp();
         uint32_t n4 = (fe - fs + 3u) & ~3u;
         if (fs + n4 > A.F) n4 = (A.F - fs) & ~3u;
         if (lane == 0 && n4) {
@@ -338,17 +340,57 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             if (dst_d) dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
             if (dst_c) dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
         }
-        if (n4) {
+        pend = n4 != 0;
+    };
+    auto wait_fill = [&]() {
+        if (pend) {
             mbar_wait(bar, parity);
             parity ^= 1u;
+            pend = false;
         }
         __syncwarp();
+    };
+    // First fill of a tile with offsets (a, b): light tile = depths and colours of all 32 lists,
+    // heavy tile = depths of its first chunk of rounds.  Issued as soon as the previous tile
+    // no longer needs the stage, i.e. BEFORE that tile's MLP, which hides the copy's latency.
+    auto chunk_end = [&](const uint32_t (&B)[L + 1], int r, uint32_t cap, uint32_t& bk) -> int {
+        int k = r + 1;                                   // greedy: rounds [r, k) fit `cap` fragments
+        bk = B[r + 1];
+#pragma unroll
+        for (int c = 1; c < L; ++c)
+            if (c > r && k == c && B[c + 1] - (B[r] & ~3u) <= cap) { k = c + 1; bk = B[c + 1]; }
+        return k;
+    };
+    auto round_bounds = [&](uint32_t a, uint32_t te, uint32_t (&B)[L + 1]) -> bool {
+#pragma unroll
+        for (int r = 0; r < L; ++r) B[r] = __shfl_sync(0xffffffffu, a, r * PPR);
+        B[L] = te;
+        bool fits = true;                                // every round fits the colour stage
+#pragma unroll
+        for (int r = 0; r < L; ++r) fits = fits && (B[r + 1] - (B[r] & ~3u) <= kCapC);
+        return fits;
+    };
+    auto first_fill = [&](uint32_t a, uint32_t b) {
+        const uint32_t tb = __shfl_sync(0xffffffffu, a, 0), te = __shfl_sync(0xffffffffu, b, 31);
+        const uint32_t fs = tb & ~3u;
+        if (te <= tb) return;
+        if (te - fs <= kCap) {
+            issue_fill(sD, sC2, fs, te);
+        } else {
+            uint32_t B[L + 1], bk;
+            if (!round_bounds(a, te, B)) return;
+            chunk_end(B, 0, kCapD, bk);
+            if (bk > B[0]) issue_fill(sD, nullptr, fs, bk);
+        }
     };
 
     uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0);
     uint32_t raw_nxt = fetch_raw();
     uint32_t o0 = 0, o1 = 0;
-    if (t_cur < A.num_tiles) load_offsets(t_cur, o0, o1);
+    if (t_cur < A.num_tiles) {
+        load_offsets(t_cur, o0, o1);
+        first_fill(o0, o1);
+    }
     while (t_cur < A.num_tiles) {
         const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
         raw_nxt = fetch_raw();
@@ -366,7 +408,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         if (te - fs <= kCap) {
             // ---- light tile: one lane per pixel, depths and colours staged together
             if (te > tb) {
-                stage_range(sD, sC2, fs, te);
+                wait_fill();                             // issued before the previous tile's MLP
                 const uint32_t first = o0 - fs, end = o1 - fs;
                 const Top2 s = scan_depths<1>(sD, first, end);
                 if (s.i1 != NOIT_ABSENT) {
@@ -387,12 +429,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             const int g = lane / L, q = lane % L;
             px_own = (uint32_t)(q * PPR + g);
             uint32_t B[L + 1];                           // fragment bounds of the rounds
-#pragma unroll
-            for (int r = 0; r < L; ++r) B[r] = __shfl_sync(0xffffffffu, o0, r * PPR);
-            B[L] = te;
-            bool fits = true;
-#pragma unroll
-            for (int r = 0; r < L; ++r) fits = fits && (B[r + 1] - (B[r] & ~3u) <= kCapC);
+            const bool fits = round_bounds(o0, te, B);
             if (!fits) {
                 own = tile_from_global<ColorT, L>(lane, o0, o1, A.depth, g_rgba);
             } else {
@@ -403,13 +440,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 #pragma unroll
                 for (int r = 0; r < L; ++r) {
                     if (r == staged_to) {                // stage the next chunk of rounds (depths)
-                        int k = r + 1;
-                        uint32_t bk = B[r + 1];
-#pragma unroll
-                        for (int c = r + 1; c < L; ++c)
-                            if (k == c && B[c + 1] - (B[r] & ~3u) <= kCapD) { k = c + 1; bk = B[c + 1]; }
+                        uint32_t bk;
+                        const int k = chunk_end(B, r, kCapD, bk);
                         const uint32_t base = B[r] & ~3u;
-                        if (bk > B[r]) stage_range(sD, nullptr, base, bk);
+                        if (r > 0 && bk > B[r]) issue_fill(sD, nullptr, base, bk);   // r == 0: first_fill
+                        wait_fill();
                         Dv = sD - base;
                         staged_to = k;
                     }
@@ -425,13 +460,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 #pragma unroll
                 for (int r = 0; r < L; ++r) {
                     if (r == staged_to) {                // stage the next chunk of rounds (colours)
-                        int k = r + 1;
-                        uint32_t bk = B[r + 1];
-#pragma unroll
-                        for (int c = r + 1; c < L; ++c)
-                            if (k == c && B[c + 1] - (B[r] & ~3u) <= kCapC) { k = c + 1; bk = B[c + 1]; }
+                        uint32_t bk;
+                        const int k = chunk_end(B, r, kCapC, bk);
                         const uint32_t base = B[r] & ~3u;
-                        if (bk > B[r]) stage_range(nullptr, sC, base, bk);
+                        if (bk > B[r]) issue_fill(nullptr, sC, base, bk);
+                        wait_fill();
                         Cv = sC - base;
                         if (q >= r && q < k) {           // owners of the chunk's rounds
                             if (t2[0].i1 != NOIT_ABSENT) {
@@ -455,6 +488,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 own.a_tail = sm[0].a; own.t_tail = sm[0].t;
             }
         }
+        // the stage is free: start the next tile's first fill, then do this tile's MLP
+        if (t_nxt < A.num_tiles) first_fill(no0, no1);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
         const uint32_t p = t_cur * 32u + px_own;
         if (p < A.P) {
