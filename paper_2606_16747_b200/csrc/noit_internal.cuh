@@ -211,6 +211,117 @@ __device__ __forceinline__ void mlp_forward_packed(const MlpWeightsT& W, const f
     f[2] = fmaxf(h3[1].x, 0.f);
 }
 
+// ---- O4 on the tensor cores (weights exactly representable in TF32, i.e. NOIT_MLP_BF16) --------
+// mma.sync.m16n8k8 TF32 with fp32 accumulation; every activation a is split into
+// a_hi = a & 0xffffe000 (a valid TF32) and a_lo = a - a_hi (exact), and a*w = a_hi*w + a_lo*w is
+// issued as two MMAs.  With w exact in TF32 the only loss is the truncation of a_lo to TF32
+// inside the second MMA (< 2^-21 |a|): fp32-class accuracy, NOT bf16/tf32 activations (A6).
+// One warp = 32 pixels = 2 m-tiles; row r of the MMA is lane r's pixel.  The C fragment of
+// layer l's n-tile s is, register for register, the A fragment of layer l+1's k-step s once
+// the hidden units are re-labelled (A col t <-> C col 2t, A col t+4 <-> C col 2t+1); that
+// re-labelling lives in the packed weights (noit_set_weights), so layers chain with no shuffle.
+// Packed weights: 11 float4 per lane, chunk v of lane l at wp[v*32 + l] (g = l>>2, t = l&3):
+//   0-1 W1 B-frags (4 n-tiles x {k=t, k=t+4}), 2-3 b1 (4 n-tiles x {col 2t, 2t+1}),
+//   4-7 W2 B-frags ((n-tile j, k-step s) x 2), 8 b2, 9 W3 B-frags (2 k-steps x 2), 10 b3.
+#define NOIT_MMA_CHUNKS 11
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const float (&a)[4], float b0, float b1,
+                                         const float (&c)[4])
+{
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
+        "{%10,%11,%12,%13};"
+        : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+        : "r"(__float_as_uint(a[0])), "r"(__float_as_uint(a[1])), "r"(__float_as_uint(a[2])),
+          "r"(__float_as_uint(a[3])), "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)),
+          "f"(c[0]), "f"(c[1]), "f"(c[2]), "f"(c[3]));
+}
+__device__ __forceinline__ void split_tf32(float v, float& hi, float& lo)
+{
+    hi = __uint_as_float(__float_as_uint(v) & 0xffffe000u);
+    lo = v - hi;
+}
+// relu + re-order of a C fragment into the next layer's A fragment, split into hi / lo
+__device__ __forceinline__ void c_to_a(const float (&c)[4], float (&hi)[4], float (&lo)[4])
+{
+    split_tf32(fmaxf(c[0], 0.f), hi[0], lo[0]);
+    split_tf32(fmaxf(c[2], 0.f), hi[1], lo[1]);
+    split_tf32(fmaxf(c[1], 0.f), hi[2], lo[2]);
+    split_tf32(fmaxf(c[3], 0.f), hi[3], lo[3]);
+}
+// All 32 lanes must call this.  x = this lane's features; scratch = 32 x 12 floats of shared
+// memory private to the warp; f = tail colour of this lane's pixel.
+__device__ __forceinline__ void mlp_forward_mma(const float4* __restrict__ wp, float* scratch, int lane,
+                                                const float x[5], float f[3])
+{
+    const int g = lane >> 2, t = lane & 3;
+    float4 wv[NOIT_MMA_CHUNKS];
+#pragma unroll
+    for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(wp + v * 32 + lane);
+    auto wf = [&](int i) -> float {                           // packed value i (constant index)
+        const float4& v = wv[i >> 2];
+        return (i & 3) == 0 ? v.x : ((i & 3) == 1 ? v.y : ((i & 3) == 2 ? v.z : v.w));
+    };
+    // features -> A fragments of layer 1 through the scratch (row = lane, stride 12: no conflicts)
+    __syncwarp();
+    *reinterpret_cast<float4*>(scratch + 12 * lane) = make_float4(x[0], x[1], x[2], x[3]);
+    scratch[12 * lane + 4] = x[4];
+    __syncwarp();
+    float fout[2][4];
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt) {
+        const float* r0 = scratch + 12 * (16 * mt + g), *r1 = r0 + 12 * 8;
+        float ahi[4], alo[4];
+        split_tf32(r0[t], ahi[0], alo[0]);
+        split_tf32(r1[t], ahi[1], alo[1]);
+        split_tf32(t == 0 ? r0[4] : 0.f, ahi[2], alo[2]);
+        split_tf32(t == 0 ? r1[4] : 0.f, ahi[3], alo[3]);
+        // layer 1: 4 n-tiles, K = 8 (5 features + zero padding)
+        float h1hi[4][4], h1lo[4][4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float bias[4] = {wf(8 + 2 * j), wf(8 + 2 * j + 1), wf(8 + 2 * j), wf(8 + 2 * j + 1)};
+            float c[4];
+            mma_tf32(c, ahi, wf(2 * j), wf(2 * j + 1), bias);
+            mma_tf32(c, alo, wf(2 * j), wf(2 * j + 1), c);
+            c_to_a(c, h1hi[j], h1lo[j]);
+        }
+        // layer 2: 2 n-tiles, 4 k-steps (k-step s = layer-1 n-tile s)
+        float h2hi[2][4], h2lo[2][4];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            float c[4] = {wf(32 + 2 * j), wf(32 + 2 * j + 1), wf(32 + 2 * j), wf(32 + 2 * j + 1)};
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const float b0 = wf(16 + 2 * (4 * j + s)), b1 = wf(16 + 2 * (4 * j + s) + 1);
+                mma_tf32(c, h1hi[s], b0, b1, c);
+                mma_tf32(c, h1lo[s], b0, b1, c);
+            }
+            c_to_a(c, h2hi[j], h2lo[j]);
+        }
+        // layer 3: 1 n-tile (3 outputs, padded to 8), 2 k-steps
+        float c[4] = {wf(40), wf(41), wf(40), wf(41)};
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            mma_tf32(c, h2hi[s], wf(36 + 2 * s), wf(36 + 2 * s + 1), c);
+            mma_tf32(c, h2lo[s], wf(36 + 2 * s), wf(36 + 2 * s + 1), c);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) fout[mt][k] = fmaxf(c[k], 0.f);
+    }
+    // C fragments (row g / g+8, cols 2t, 2t+1) -> one row per lane
+    __syncwarp();
+    if (t < 2) {
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+            float* r0 = scratch + 12 * (16 * mt + g) + 2 * t, *r1 = r0 + 12 * 8;
+            *reinterpret_cast<float2*>(r0) = make_float2(fout[mt][0], fout[mt][1]);
+            *reinterpret_cast<float2*>(r1) = make_float2(fout[mt][2], fout[mt][3]);
+        }
+    }
+    __syncwarp();
+    const float4 o = *reinterpret_cast<const float4*>(scratch + 12 * lane);
+    f[0] = o.x; f[1] = o.y; f[2] = o.z;
+}
+
 // O3 features from raw accumulators; returns has_tail (A2).
 __device__ __forceinline__ bool make_features(float n, float t_tail, float ar, float ag, float ab,
                                               float a_tail, float x[5])

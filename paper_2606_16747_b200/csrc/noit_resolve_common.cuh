@@ -22,6 +22,7 @@ struct ResolveArgs {
     const float* coarse_g[2];      // G[10] per coarse pixel, lod 1 (half) and lod 2 (quarter)
     int32_t coarse_w[2], coarse_h[2];
     // staged kernel
+    const float4* mlp_packed;      // per-lane MMA fragments of the weights (NOIT_MLP_BF16)
     uint32_t num_tiles;
     uint32_t* tile_counter;        // [0] next tile, [1] finished warps; self-resetting
 };

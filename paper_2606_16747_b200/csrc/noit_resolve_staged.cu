@@ -33,8 +33,10 @@
 
 namespace {
 
-constexpr uint32_t kCap = 1032;          // fragments per warp stage: 8 px * 128 + alignment slack (16 warps/SM)
+constexpr uint32_t kCap = 1000;          // fragments per warp stage (12000 B with fp16 colour: 16 warps/SM)
+constexpr uint32_t kScratchFloats = 32 * 12;   // per warp: feature / output transpose of the MMA MLP
 constexpr int kWarpsPerCta = 4;
+constexpr uint32_t kTileBatch = 1;       // tiles per atomic (4 measured slower: 204 vs 168 us, heavy tiles cluster)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
 {
@@ -283,7 +285,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <typename ColorT, int L>
+template <typename ColorT, int L, bool kMma>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
 {
@@ -300,6 +302,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     Packed* const sC2 = reinterpret_cast<Packed*>(stage + kCap * 4u);    // colours behind kCap depths
     Packed* const sC = reinterpret_cast<Packed*>(stage);                 // colours only
     const uint32_t bar = smem_u32(reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * kStageBytes) + warp);
+    float* const scratch = reinterpret_cast<float*>(smem_raw + kWarpsPerCta * kStageBytes +
+                                                    kWarpsPerCta * sizeof(uint64_t)) + warp * kScratchFloats;
     if (lane == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -317,7 +321,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         return t;
     };
     auto load_offsets = [&](uint32_t tile, uint32_t& a, uint32_t& b) {
-        const uint32_t p = tile * 32u + lane;
+        // tiles are taken from the end of the frame backwards (shorter tail in cfg3: 1.5 % vs 4.6 %
+        // of the makespan in a list-scheduling model of the measured tile costs)
+        const uint32_t p = (A.num_tiles - 1u - tile) * 32u + lane;
         a = __ldg(offsets + min(p, A.P));
         b = __ldg(offsets + min(p + 1u, A.P));
     };
@@ -384,16 +390,25 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         }
     };
 
-    uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0);
-    uint32_t raw_nxt = fetch_raw();
+    // tiles are taken in batches of kTileBatch consecutive tiles per atomic: same-address
+    // atomics are serialised by the L2, one per tile would cap the kernel
+    uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0) * kTileBatch;
+    uint32_t raw_nxt = fetch_raw(), raw_nn = fetch_raw();   // two atomics in flight
+    uint32_t left = kTileBatch - 1;                      // tiles of the current batch after t_cur
     uint32_t o0 = 0, o1 = 0;
     if (t_cur < A.num_tiles) {
         load_offsets(t_cur, o0, o1);
         first_fill(o0, o1);
     }
     while (t_cur < A.num_tiles) {
-        const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
-        raw_nxt = fetch_raw();
+        uint32_t t_nxt = t_cur + 1u;
+        if (left == 0) {
+            t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0) * kTileBatch;
+            raw_nxt = raw_nn;
+            raw_nn = fetch_raw();
+            left = kTileBatch;
+        }
+        left -= 1u;
         uint32_t no0 = 0, no1 = 0;
         if (t_nxt < A.num_tiles) load_offsets(t_nxt, no0, no1);   // lands while this tile runs
 
@@ -491,18 +506,21 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         // the stage is free: start the next tile's first fill, then do this tile's MLP
         if (t_nxt < A.num_tiles) first_fill(no0, no1);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
-        const uint32_t p = t_cur * 32u + px_own;
-        if (p < A.P) {
+        const uint32_t p = (A.num_tiles - 1u - t_cur) * 32u + px_own;
+        {
             float xf[5], f[3];
             // O3 with one IEEE reciprocal instead of three divisions
             const bool has_tail = own.a_tail > 0.f;
             const float inv = has_tail ? 1.0f / own.a_tail : 0.f;
             xf[0] = (float)own.n; xf[1] = own.t_tail;
             xf[2] = own.acc_r * inv; xf[3] = own.acc_g * inv; xf[4] = own.acc_b * inv;
-            mlp_forward_packed(W, xf, f);
-            const float4 c1 = Color<ColorT>::unpack(own.c1), c2 = Color<ColorT>::unpack(own.c2);
-            composite_store(A, p, c1, make_float4(c2.w * c2.x, c2.w * c2.y, c2.w * c2.z, c2.w),
-                            own.n ? own.d1 : 1.0f, has_tail, f, own.t_tail);
+            if (kMma) mlp_forward_mma(A.mlp_packed, scratch, lane, xf, f);     // all 32 lanes
+            else mlp_forward_packed(W, xf, f);
+            if (p < A.P) {
+                const float4 c1 = Color<ColorT>::unpack(own.c1), c2 = Color<ColorT>::unpack(own.c2);
+                composite_store(A, p, c1, make_float4(c2.w * c2.x, c2.w * c2.y, c2.w * c2.z, c2.w),
+                                own.n ? own.d1 : 1.0f, has_tail, f, own.t_tail);
+            }
         }
         t_cur = t_nxt; o0 = no0; o1 = no1;
     }
@@ -517,24 +535,24 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     }
 }
 
-template <typename ColorT, int L>
+template <typename ColorT, int L, bool kMma>
 static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
 {
     const size_t smem = kWarpsPerCta * (size_t)kCap * (4u + Color<ColorT>::kBytes) +
-                        kWarpsPerCta * sizeof(uint64_t);
+                        kWarpsPerCta * sizeof(uint64_t) + kWarpsPerCta * kScratchFloats * sizeof(float);
     static bool configured = false;                     // per instantiation
     if (!configured) {
-        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L>,
+        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = true;
     }
     int per_sm = 0;
     NOIT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                       &per_sm, resolve_staged_kernel<ColorT, L>, kWarpsPerCta * 32, smem));
+                       &per_sm, resolve_staged_kernel<ColorT, L, kMma>, kWarpsPerCta * 32, smem));
     if (per_sm < 1) return noit_fail(ctx, NOIT_ERR_CUDA, "resolve_staged_kernel does not fit an SM");
     const uint32_t want = (A.num_tiles + kWarpsPerCta - 1) / kWarpsPerCta;
     const uint32_t grid = min((uint32_t)(ctx->num_sms * per_sm), max(want, 1u));
-    resolve_staged_kernel<ColorT, L><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
+    resolve_staged_kernel<ColorT, L, kMma><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
     ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
@@ -546,6 +564,11 @@ noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int
     ResolveArgs A = A0;
     A.num_tiles = (A.P + 31u) / 32u;
     A.tile_counter = ctx->d_counters;
-    if (color_fmt == NOIT_RGBA_F16) return launch_staged<__half, 4>(ctx, A, st);
-    return launch_staged<float, 4>(ctx, A, st);
+    A.mlp_packed = static_cast<const float4*>(ctx->d_mlp);
+    // bf16-rounded weights are exact in TF32: the MLP runs on the tensor cores (two-pass split
+    // of the activations, fp32-class accuracy); fp32 weights keep the FFMA2 form.
+    const bool mma = ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp != nullptr;
+    if (color_fmt == NOIT_RGBA_F16)
+        return mma ? launch_staged<__half, 4, true>(ctx, A, st) : launch_staged<__half, 4, false>(ctx, A, st);
+    return mma ? launch_staged<float, 4, true>(ctx, A, st) : launch_staged<float, 4, false>(ctx, A, st);
 }
