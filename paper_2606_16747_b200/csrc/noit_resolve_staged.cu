@@ -292,8 +292,10 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     typedef typename Color<ColorT>::Packed Packed;
     constexpr uint32_t CB = Color<ColorT>::kBytes;
     constexpr uint32_t kStageBytes = kCap * (4u + CB);   // per warp
-    constexpr uint32_t kCapD = kStageBytes / 4u;         // fragments when the stage holds depths only
-    constexpr uint32_t kCapC = kStageBytes / CB;         // ... colours only
+    // fragments when the stage holds depths only / colours only; multiples of 4 because a copy
+    // is rounded up to 4 fragments
+    constexpr uint32_t kCapD = (kStageBytes / 4u) & ~3u;
+    constexpr uint32_t kCapC = (kStageBytes / CB) & ~3u;
     constexpr int PPR = 32 / L;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -301,9 +303,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     float* const sD = reinterpret_cast<float*>(stage);                   // depths (both views)
     Packed* const sC2 = reinterpret_cast<Packed*>(stage + kCap * 4u);    // colours behind kCap depths
     Packed* const sC = reinterpret_cast<Packed*>(stage);                 // colours only
-    const uint32_t bar = smem_u32(reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * kStageBytes) + warp);
-    float* const scratch = reinterpret_cast<float*>(smem_raw + kWarpsPerCta * kStageBytes +
-                                                    kWarpsPerCta * sizeof(uint64_t)) + warp * kScratchFloats;
+    // layout: stages | scratch (16-byte aligned rows) | mbarriers
+    float* const scratch = reinterpret_cast<float*>(smem_raw + kWarpsPerCta * kStageBytes) + warp * kScratchFloats;
+    const uint32_t bar = smem_u32(reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * kStageBytes +
+                                                              kWarpsPerCta * kScratchFloats * sizeof(float)) + warp);
+    static_assert(kStageBytes % 16 == 0 && (kCap * 4u) % 16 == 0, "bulk copies need 16-byte aligned destinations");
     if (lane == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

@@ -160,6 +160,28 @@ def test_resolve_random_ragged(noit, dtype, precision, seed, shape):
     check_resolve(noit, fbh, w, precision, got)
 
 
+@pytest.mark.parametrize("dtype,lo,hi", [
+    (np.float16, 100, 128), (np.float32, 100, 128), (np.float16, 180, 188), (np.float32, 150, 157),
+    (np.float16, 60, 70), (np.float32, 36, 40), (np.float16, 28, 32)])
+def test_resolve_dense_tiles(noit, dtype, lo, hi):
+    """Every tile near a staging boundary of the staged kernel: whole-tile stage, depth-only
+    chunks of 4 / 2 rounds, colour chunks of 2 / 1 rounds, rounds that barely fit or do not."""
+    rng = np.random.default_rng(lo * 1000 + hi)
+    W, H = 96, 5
+    counts = rng.integers(lo, hi + 1, W * H)
+    off = np.zeros(W * H + 1, np.uint32)
+    off[1:] = np.cumsum(counts)
+    F = int(off[-1])
+    depth = rng.uniform(0.01, 0.99, F).astype(np.float32)
+    ties = rng.random(F) < 0.2
+    depth[ties] = rng.choice(np.asarray([0.125, 0.5], np.float32), int(ties.sum()))
+    fbh = FragBuf(W, H, off, depth, rng.uniform(0, 1, (F, 4)).astype(dtype))
+    w = noit_scenes.mlp_weights(7)
+    ctx = noit.Noit(w, 1)
+    got = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
+    check_resolve(noit, fbh, w, 1, got)
+
+
 def test_resolve_empty_and_single_output(noit):
     w = noit_scenes.mlp_weights(0)
     ctx = noit.Noit(w, 0)
