@@ -1,89 +1,10 @@
-// noit_resolve.cu -- noit_resolve / noit_resolve_host: host-side checks and dispatch, plus the
-// GENERAL resolve kernel (one pixel per thread, fragments read straight from global memory).
-// The general kernel serves S9 (scattered pixel list) and S7 (adaptive, per-tile LOD); plain
-// frames go to the staged kernel (noit_resolve_staged.cu).
+// noit_resolve.cu -- noit_resolve / noit_resolve_host: host-side checks and dispatch, and the S7
+// pre-pass (coarse_g_kernel).  Every resolve (plain frame, S7 adaptive, S9 pixel list) runs in
+// the staged kernel (noit_resolve_staged.cu).
 #include "noit_resolve_common.cuh"
 
-noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt,
+noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt, int mode,
                                        cudaStream_t st);
-
-enum { MODE_ALL = 0, MODE_LIST = 1, MODE_ADAPTIVE = 2 };
-
-// lod > 0 pixel of S7 (O7): bilinear sample of G = [a2*C2 (3), a2, C_acc (3), A_tail, T_tail, N]
-// at the full-res pixel centre, taps clamped to the coarse texels of the pixel's own leaf and to
-// the image (A19).  lerp(a,b,w) = a + w(b-a), x first then y; the weights are dyadic.
-__device__ __forceinline__ void sample_coarse_g(const float* __restrict__ G, int cw, int ch, int r,
-                                                int leaf_side, int x, int y, float out[10])
-{
-    const float inv_r = 1.f / (float)r;
-    const float u = ((float)x + 0.5f) * inv_r - 0.5f, v = ((float)y + 0.5f) * inv_r - 0.5f;
-    const float fu = floorf(u), fv = floorf(v);
-    const int i0 = (int)fu, j0 = (int)fv;
-    const float wx = u - fu, wy = v - fv;
-    const int lx0 = (x / leaf_side) * leaf_side, ly0 = (y / leaf_side) * leaf_side;
-    const int tx_lo = lx0 / r, ty_lo = ly0 / r;
-    const int tx_hi = min((lx0 + leaf_side - 1) / r, cw - 1);
-    const int ty_hi = min((ly0 + leaf_side - 1) / r, ch - 1);
-    const int xa = min(max(i0, tx_lo), tx_hi), xb = min(max(i0 + 1, tx_lo), tx_hi);
-    const int ya = min(max(j0, ty_lo), ty_hi), yb = min(max(j0 + 1, ty_lo), ty_hi);
-    const float* g00 = G + 10 * ((size_t)ya * cw + xa);
-    const float* g10 = G + 10 * ((size_t)ya * cw + xb);
-    const float* g01 = G + 10 * ((size_t)yb * cw + xa);
-    const float* g11 = G + 10 * ((size_t)yb * cw + xb);
-#pragma unroll
-    for (int k = 0; k < 10; ++k) {
-        const float a = g00[k], b = g10[k], c = g01[k], d = g11[k];
-        const float top = fmaf(wx, b - a, a), bot = fmaf(wx, d - c, c);
-        out[k] = fmaf(wy, bot - top, top);
-    }
-}
-
-template <typename ColorT, int kMode>
-__global__ void __launch_bounds__(128)
-resolve_general_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeights W)
-{
-    const ColorT* __restrict__ rgba = static_cast<const ColorT*>(A.rgba);
-    const uint32_t stride = gridDim.x * blockDim.x;
-    const uint32_t total = kMode == MODE_LIST ? min(__ldg(A.pixel_count), A.P) : A.P;
-    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += stride) {
-        const uint32_t p = kMode == MODE_LIST ? __ldg(A.pixel_list + t) : t;
-        const uint32_t b = __ldg(A.offsets + p), e = __ldg(A.offsets + p + 1);
-        int lod = 0, level = 3, x = 0, y = 0;
-        if (kMode == MODE_ADAPTIVE) {
-            y = (int)(p / (uint32_t)A.W);
-            x = (int)(p - (uint32_t)y * (uint32_t)A.W);
-            level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)];
-            lod = A.level_to_lod[level & 3];
-        }
-        float xf[5], f[3];
-        if (kMode != MODE_ADAPTIVE || lod == 0) {
-            PixelState<false> s;
-            s.init();
-            for (uint32_t j = b; j < e; ++j) s.push(__ldg(A.depth + j), load_rgba(rgba, j), j);
-            const bool has_tail = make_features((float)(e - b), s.t_tail, s.acc_r, s.acc_g,
-                                                s.acc_b, s.a_tail, xf);
-            mlp_forward(W, xf, f);
-            const float4 l2 = make_float4(s.c2.w * s.c2.x, s.c2.w * s.c2.y, s.c2.w * s.c2.z, s.c2.w);
-            composite_store(A, p, s.c1, l2, e > b ? s.d1 : 1.0f, has_tail, f, s.t_tail);
-        } else {
-            // layer 1 from the FULL buffer: depth-only scan, then one colour fetch
-            float d1 = __int_as_float(0x7f800000);
-            uint32_t i1 = b;
-            for (uint32_t j = b; j < e; ++j) {
-                const float d = __ldg(A.depth + j);
-                if (d < d1) { d1 = d; i1 = j; }
-            }
-            float4 c1 = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (e > b) c1 = load_rgba(rgba, i1); else d1 = 1.0f;
-            float G[10];
-            sample_coarse_g(A.coarse_g[lod - 1], A.coarse_w[lod - 1], A.coarse_h[lod - 1], 1 << lod,
-                            64 >> level, x, y, G);
-            const bool has_tail = make_features(G[9], G[8], G[4], G[5], G[6], G[7], xf);
-            mlp_forward(W, xf, f);
-            composite_store(A, p, c1, make_float4(G[0], G[1], G[2], G[3]), d1, has_tail, f, G[8]);
-        }
-    }
-}
 
 // S7 pre-pass: G[10] of every coarse pixel whose leaf is resolved at this lod (self-contained
 // O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
@@ -146,16 +67,6 @@ static noit_status check_desc(noit_ctx* ctx, const noit_resolve_desc* d, const c
     return NOIT_OK;
 }
 
-template <int kMode>
-static void launch_general(const ResolveArgs& A, const MlpWeights& W, int fmt, uint32_t blocks,
-                           cudaStream_t st)
-{
-    if (fmt == NOIT_RGBA_F16)
-        resolve_general_kernel<__half, kMode><<<blocks, 128, 0, st>>>(A, W);
-    else
-        resolve_general_kernel<float, kMode><<<blocks, 128, 0, st>>>(A, W);
-}
-
 static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cudaStream_t st)
 {
     ResolveArgs A;
@@ -176,12 +87,8 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
     A.cell_level = d->cell_level;
     const int fmt = d->full.color_fmt;
 
-    if (d->pixel_list) {                                   // S9
-        launch_general<MODE_LIST>(A, ctx->w, fmt, (uint32_t)ctx->num_sms * 8, st);
-        ctx->launches += 1;
-        NOIT_CUDA(ctx, cudaGetLastError());
-        return NOIT_OK;
-    }
+    if (d->pixel_list)                                     // S9: staged kernel, list mode
+        return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_LIST, st);
     if (d->cell_level) {                                   // S7
         memcpy(A.level_to_lod, d->level_to_lod, 4);
         const uchar4 l2l = make_uchar4(d->level_to_lod[0], d->level_to_lod[1], d->level_to_lod[2],
@@ -217,12 +124,9 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
         }
-        launch_general<MODE_ADAPTIVE>(A, ctx->w, fmt, (A.P + 127) / 128, st);
-        ctx->launches += 1;
-        NOIT_CUDA(ctx, cudaGetLastError());
-        return NOIT_OK;
+        return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_ADAPTIVE, st);
     }
-    return noit_launch_resolve_staged(ctx, A, fmt, st);     // plain frame: staged kernel
+    return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_ALL, st);
 }
 
 extern "C" {

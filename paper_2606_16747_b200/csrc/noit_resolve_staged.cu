@@ -238,7 +238,7 @@ __device__ __forceinline__ void transposed_sum(Sums (&s)[L], int q)
 
 // ---- cold path: a tile with a round too long for the stage (lists far beyond BASELINE.json's
 // 128-fragment cap) reads global memory directly; the two layers are skipped by index in pass 2.
-template <typename ColorT, int L>
+template <typename ColorT, int L, int kRounds>
 __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, uint32_t o1,
                                                        const float* __restrict__ depth,
                                                        const typename Color<ColorT>::Packed* __restrict__ rgba)
@@ -246,21 +246,32 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
     constexpr int PPR = 32 / L;
     const int g = lane / L, q = lane % L;
     Owned<ColorT> own;
-    for (int r = 0; r < L; ++r) {
+    own.c1 = own.c2 = Color<ColorT>::zero();
+    own.d1 = 1.0f; own.n = 0;
+    own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
+    for (int r = 0; r < kRounds; ++r) {
         const int px = r * PPR + g;
         const uint32_t b = __shfl_sync(0xffffffffu, o0, px), e = __shfl_sync(0xffffffffu, o1, px);
         Top2 s;
         s.d1 = s.d2 = __int_as_float(0x7f800000);
         s.i1 = s.i2 = NOIT_ABSENT;
-        for (uint32_t j = b + q; j < e; j += L) top2_push(s, __ldg(depth + j), j);
+        // latency-bound (scattered lists): four loads in flight per lane, and the colours are
+        // pulled into L2 while the depths are scanned
+#pragma unroll 4
+        for (uint32_t j = b + q; j < e; j += L) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(rgba + j));
+            top2_push(s, __ldg(depth + j), j);
+        }
 #pragma unroll
         for (int m = 1; m < L; m <<= 1)
             top2_merge(s, __shfl_xor_sync(0xffffffffu, s.d1, m), __shfl_xor_sync(0xffffffffu, s.i1, m),
                        __shfl_xor_sync(0xffffffffu, s.d2, m), __shfl_xor_sync(0xffffffffu, s.i2, m));
         float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f;
+#pragma unroll 4
         for (uint32_t j = b + q; j < e; j += L) {
-            if (j == s.i1 || j == s.i2) continue;
-            const float4 c = Color<ColorT>::unpack(__ldg(rgba + j));
+            typename Color<ColorT>::Packed raw = __ldg(rgba + j);
+            if (j == s.i1 || j == s.i2) raw = Color<ColorT>::zero_alpha_reg(raw);
+            const float4 c = Color<ColorT>::unpack(raw);
             ar = fmaf(c.w, c.x, ar); ag = fmaf(c.w, c.y, ag); ab = fmaf(c.w, c.z, ab);
             at += c.w;
             tt = fmaf(-c.w, tt, tt);
@@ -285,7 +296,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <typename ColorT, int L, bool kMma>
+template <typename ColorT, int L, bool kMma, int kMode>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
 {
@@ -324,12 +335,36 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         if (lane == 0) t = atomicAdd(A.tile_counter, 1u);
         return t;
     };
-    auto load_offsets = [&](uint32_t tile, uint32_t& a, uint32_t& b) {
-        // tiles are taken from the end of the frame backwards (shorter tail in cfg3: 1.5 % vs 4.6 %
-        // of the makespan in a list-scheduling model of the measured tile costs)
-        const uint32_t p = (A.num_tiles - 1u - tile) * 32u + lane;
-        a = __ldg(offsets + min(p, A.P));
-        b = __ldg(offsets + min(p + 1u, A.P));
+    // S9 (kMode LIST): "tile" t = entries [t*32/L, (t+1)*32/L) of the pixel list; the lists of a
+    // tile are not contiguous, so such tiles always take the global path.
+    const uint32_t list_total = kMode == NOIT_RESOLVE_LIST ? min(__ldg(A.pixel_count), A.P) : 0u;
+    const uint32_t num_tiles = kMode == NOIT_RESOLVE_LIST ? (list_total + PPR - 1u) / PPR : A.num_tiles;
+    // pixel index this lane loads the offsets of (kMode ALL / ADAPTIVE: tiles are taken from the
+    // end of the frame backwards -- shorter tail in cfg3: 1.5 % vs 4.6 % of the makespan in a
+    // list-scheduling model of the measured tile costs)
+    auto lane_pixel = [&](uint32_t tile) -> uint32_t {
+        if constexpr (kMode == NOIT_RESOLVE_LIST) {
+            const uint32_t i = tile * PPR + (lane % PPR);        // lanes 0..PPR-1 hold the entries
+            return i < list_total ? __ldg(A.pixel_list + i) : 0xFFFFFFFFu;
+        }
+        return (num_tiles - 1u - tile) * 32u + lane;
+    };
+    auto load_offsets = [&](uint32_t pix, uint32_t& a, uint32_t& b) {
+        if (kMode == NOIT_RESOLVE_LIST) {
+            a = pix < A.P ? __ldg(offsets + pix) : 0u;
+            b = pix < A.P ? __ldg(offsets + pix + 1u) : a;
+        } else {
+            a = __ldg(offsets + min(pix, A.P));
+            b = __ldg(offsets + min(pix + 1u, A.P));
+        }
+    };
+    // S7 (kMode ADAPTIVE): lod of the lane's pixel; a tile with any lod > 0 takes the mixed path
+    auto lane_lod = [&](uint32_t pix, int& level) -> int {
+        level = 3;
+        if (kMode != NOIT_RESOLVE_ADAPTIVE || pix >= A.P) return 0;
+        const uint32_t y = pix / (uint32_t)A.W, x = pix - y * (uint32_t)A.W;
+        level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)] & 3;
+        return A.level_to_lod[level];
     };
     // Issue the copy of fragments [fs, fe) (fs a multiple of 4 = 16 bytes) into the stage; the
     // caller has made sure nobody still reads the old contents.  The bulk copies never read
@@ -380,7 +415,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         for (int r = 0; r < L; ++r) fits = fits && (B[r + 1] - (B[r] & ~3u) <= kCapC);
         return fits;
     };
-    auto first_fill = [&](uint32_t a, uint32_t b) {
+    auto first_fill = [&](uint32_t a, uint32_t b, bool unstaged) {
+        if (kMode == NOIT_RESOLVE_LIST || unstaged) return;
         const uint32_t tb = __shfl_sync(0xffffffffu, a, 0), te = __shfl_sync(0xffffffffu, b, 31);
         const uint32_t fs = tb & ~3u;
         if (te <= tb) return;
@@ -399,12 +435,17 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0) * kTileBatch;
     uint32_t raw_nxt = fetch_raw(), raw_nn = fetch_raw();   // two atomics in flight
     uint32_t left = kTileBatch - 1;                      // tiles of the current batch after t_cur
-    uint32_t o0 = 0, o1 = 0;
-    if (t_cur < A.num_tiles) {
-        load_offsets(t_cur, o0, o1);
-        first_fill(o0, o1);
+    uint32_t o0 = 0, o1 = 0, pix = 0;
+    int lod = 0, level = 3;
+    bool mixed = false;                                  // S7: the tile has pixels with lod > 0
+    if (t_cur < num_tiles) {
+        pix = lane_pixel(t_cur);
+        load_offsets(pix, o0, o1);
+        lod = lane_lod(pix, level);
+        mixed = __any_sync(0xffffffffu, lod > 0);
+        first_fill(o0, o1, mixed);
     }
-    while (t_cur < A.num_tiles) {
+    while (t_cur < num_tiles) {
         uint32_t t_nxt = t_cur + 1u;
         if (left == 0) {
             t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0) * kTileBatch;
@@ -413,8 +454,15 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             left = kTileBatch;
         }
         left -= 1u;
-        uint32_t no0 = 0, no1 = 0;
-        if (t_nxt < A.num_tiles) load_offsets(t_nxt, no0, no1);   // lands while this tile runs
+        uint32_t no0 = 0, no1 = 0, npix = 0;
+        int nlod = 0, nlevel = 3;
+        bool nmixed = false;
+        if (t_nxt < num_tiles) {                         // lands while this tile runs
+            npix = lane_pixel(t_nxt);
+            load_offsets(npix, no0, no1);
+            nlod = lane_lod(npix, nlevel);
+            nmixed = __any_sync(0xffffffffu, nlod > 0);
+        }
 
         Owned<ColorT> own;
         own.c1 = own.c2 = Color<ColorT>::zero();
@@ -422,9 +470,54 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
         uint32_t px_own = lane;                          // pixel of the tile this lane ends up owning
 
+        // inputs of the epilogue when a path produces them directly (S7 mixed tiles)
+        float xf[5];
+        float4 e_c1 = make_float4(0.f, 0.f, 0.f, 0.f), e_l2 = e_c1;
+        float e_d1 = 1.0f, e_tt = 1.0f;
+        bool has_tail = false, epi_ready = false;
+
         const uint32_t tb = __shfl_sync(0xffffffffu, o0, 0), te = __shfl_sync(0xffffffffu, o1, 31);
         const uint32_t fs = tb & ~3u;
-        if (te - fs <= kCap) {
+        if (kMode == NOIT_RESOLVE_LIST) {
+            // ---- S9: 32/L scattered pixels, L lanes per pixel straight from global memory (one
+            // round: the lists are scattered, so the work is latency-bound and small tiles keep
+            // every warp of the machine busy); lanes with lane % L == 0 own a pixel
+            px_own = (uint32_t)(lane / L);
+            own = tile_from_global<ColorT, L, 1>(lane, o0, o1, A.depth, g_rgba);
+        } else if (kMode == NOIT_RESOLVE_ADAPTIVE && mixed) {
+            // ---- S7 tile with coarse pixels (smooth regions: few fragments): one lane per pixel
+            // straight from global memory.  lod 0 lanes: O1-O3; lod > 0 lanes: layer 1 from the
+            // full buffer (depth-only scan + one colour fetch), layer 2 and the raw tail
+            // accumulators bilinearly sampled from the coarse buffer's G (O7).
+            const ColorT* rgba_t = static_cast<const ColorT*>(A.rgba);
+            epi_ready = true;
+            if (lod == 0) {
+                PixelState<false> ps;
+                ps.init();
+                for (uint32_t j = o0; j < o1; ++j) ps.push(__ldg(A.depth + j), load_rgba(rgba_t, j), j);
+                has_tail = make_features((float)(o1 - o0), ps.t_tail, ps.acc_r, ps.acc_g, ps.acc_b,
+                                         ps.a_tail, xf);
+                e_c1 = ps.c1;
+                e_l2 = make_float4(ps.c2.w * ps.c2.x, ps.c2.w * ps.c2.y, ps.c2.w * ps.c2.z, ps.c2.w);
+                e_d1 = o1 > o0 ? ps.d1 : 1.0f;
+                e_tt = ps.t_tail;
+            } else {
+                float d1 = __int_as_float(0x7f800000);
+                uint32_t i1 = o0;
+                for (uint32_t j = o0; j < o1; ++j) {
+                    const float d = __ldg(A.depth + j);
+                    if (d < d1) { d1 = d; i1 = j; }
+                }
+                if (o1 > o0) { e_c1 = load_rgba(rgba_t, i1); e_d1 = d1; }
+                const int y = (int)(pix / (uint32_t)A.W), x = (int)(pix - (uint32_t)y * (uint32_t)A.W);
+                float G[10];
+                sample_coarse_g(A.coarse_g[lod - 1], A.coarse_w[lod - 1], A.coarse_h[lod - 1], 1 << lod,
+                                64 >> level, x, y, G);
+                has_tail = make_features(G[9], G[8], G[4], G[5], G[6], G[7], xf);
+                e_l2 = make_float4(G[0], G[1], G[2], G[3]);
+                e_tt = G[8];
+            }
+        } else if (te - fs <= kCap) {
             // ---- light tile: one lane per pixel, depths and colours staged together
             if (te > tb) {
                 wait_fill();                             // issued before the previous tile's MLP
@@ -450,7 +543,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             uint32_t B[L + 1];                           // fragment bounds of the rounds
             const bool fits = round_bounds(o0, te, B);
             if (!fits) {
-                own = tile_from_global<ColorT, L>(lane, o0, o1, A.depth, g_rgba);
+                own = tile_from_global<ColorT, L, L>(lane, o0, o1, A.depth, g_rgba);
             } else {
                 Top2 t2[L];
                 uint32_t first[L], end[L];
@@ -508,24 +601,29 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             }
         }
         // the stage is free: start the next tile's first fill, then do this tile's MLP
-        if (t_nxt < A.num_tiles) first_fill(no0, no1);
+        if (t_nxt < num_tiles) first_fill(no0, no1, nmixed);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
-        const uint32_t p = (A.num_tiles - 1u - t_cur) * 32u + px_own;
+        uint32_t p = __shfl_sync(0xffffffffu, pix, (int)px_own);
+        if (kMode == NOIT_RESOLVE_LIST && (lane % L) != 0) p = 0xFFFFFFFFu;   // not an owner
         {
-            float xf[5], f[3];
-            // O3 with one IEEE reciprocal instead of three divisions
-            const bool has_tail = own.a_tail > 0.f;
-            const float inv = has_tail ? 1.0f / own.a_tail : 0.f;
-            xf[0] = (float)own.n; xf[1] = own.t_tail;
-            xf[2] = own.acc_r * inv; xf[3] = own.acc_g * inv; xf[4] = own.acc_b * inv;
+            float f[3];
+            if (!epi_ready) {
+                // O3 with one IEEE reciprocal instead of three divisions
+                has_tail = own.a_tail > 0.f;
+                const float inv = has_tail ? 1.0f / own.a_tail : 0.f;
+                xf[0] = (float)own.n; xf[1] = own.t_tail;
+                xf[2] = own.acc_r * inv; xf[3] = own.acc_g * inv; xf[4] = own.acc_b * inv;
+                const float4 c2 = Color<ColorT>::unpack(own.c2);
+                e_c1 = Color<ColorT>::unpack(own.c1);
+                e_l2 = make_float4(c2.w * c2.x, c2.w * c2.y, c2.w * c2.z, c2.w);
+                e_d1 = own.n ? own.d1 : 1.0f;
+                e_tt = own.t_tail;
+            }
             if (kMma) mlp_forward_mma(A.mlp_packed, scratch, lane, xf, f);     // all 32 lanes
             else mlp_forward_packed(W, xf, f);
-            if (p < A.P) {
-                const float4 c1 = Color<ColorT>::unpack(own.c1), c2 = Color<ColorT>::unpack(own.c2);
-                composite_store(A, p, c1, make_float4(c2.w * c2.x, c2.w * c2.y, c2.w * c2.z, c2.w),
-                                own.n ? own.d1 : 1.0f, has_tail, f, own.t_tail);
-            }
+            if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
+        pix = npix; lod = nlod; level = nlevel; mixed = nmixed;
         t_cur = t_nxt; o0 = no0; o1 = no1;
     }
     // the last warp to finish re-arms the counters for the next launch
@@ -539,40 +637,58 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     }
 }
 
-template <typename ColorT, int L, bool kMma>
+template <typename ColorT, int L, bool kMma, int kMode>
 static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
 {
     const size_t smem = kWarpsPerCta * (size_t)kCap * (4u + Color<ColorT>::kBytes) +
                         kWarpsPerCta * sizeof(uint64_t) + kWarpsPerCta * kScratchFloats * sizeof(float);
     static bool configured = false;                     // per instantiation
     if (!configured) {
-        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma>,
+        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma, kMode>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = true;
     }
     int per_sm = 0;
     NOIT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                       &per_sm, resolve_staged_kernel<ColorT, L, kMma>, kWarpsPerCta * 32, smem));
+                       &per_sm, resolve_staged_kernel<ColorT, L, kMma, kMode>, kWarpsPerCta * 32, smem));
     if (per_sm < 1) return noit_fail(ctx, NOIT_ERR_CUDA, "resolve_staged_kernel does not fit an SM");
-    const uint32_t want = (A.num_tiles + kWarpsPerCta - 1) / kWarpsPerCta;
+    // S9 reads its tile count on the device: the persistent grid is sized for the machine
+    const uint32_t want = kMode == NOIT_RESOLVE_LIST ? 0xFFFFFFFFu
+                                                     : (A.num_tiles + kWarpsPerCta - 1) / kWarpsPerCta;
     const uint32_t grid = min((uint32_t)(ctx->num_sms * per_sm), max(want, 1u));
-    resolve_staged_kernel<ColorT, L, kMma><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
+    resolve_staged_kernel<ColorT, L, kMma, kMode><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
     ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
 }
 
-noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int color_fmt,
+template <typename ColorT, int kMode>
+static noit_status launch_mode(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
+{
+    // bf16-rounded weights are exact in TF32: the MLP runs on the tensor cores (two-pass split
+    // of the activations, fp32-class accuracy); fp32 weights keep the FFMA2 form.
+    const bool mma = ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp != nullptr;
+    return mma ? launch_staged<ColorT, 4, true, kMode>(ctx, A, st)
+               : launch_staged<ColorT, 4, false, kMode>(ctx, A, st);
+}
+
+noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int color_fmt, int mode,
                                        cudaStream_t st)
 {
     ResolveArgs A = A0;
     A.num_tiles = (A.P + 31u) / 32u;
     A.tile_counter = ctx->d_counters;
     A.mlp_packed = static_cast<const float4*>(ctx->d_mlp);
-    // bf16-rounded weights are exact in TF32: the MLP runs on the tensor cores (two-pass split
-    // of the activations, fp32-class accuracy); fp32 weights keep the FFMA2 form.
-    const bool mma = ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp != nullptr;
-    if (color_fmt == NOIT_RGBA_F16)
-        return mma ? launch_staged<__half, 4, true>(ctx, A, st) : launch_staged<__half, 4, false>(ctx, A, st);
-    return mma ? launch_staged<float, 4, true>(ctx, A, st) : launch_staged<float, 4, false>(ctx, A, st);
+    const bool f16 = color_fmt == NOIT_RGBA_F16;
+    switch (mode) {
+    case NOIT_RESOLVE_LIST:
+        return f16 ? launch_mode<__half, NOIT_RESOLVE_LIST>(ctx, A, st)
+                   : launch_mode<float, NOIT_RESOLVE_LIST>(ctx, A, st);
+    case NOIT_RESOLVE_ADAPTIVE:
+        return f16 ? launch_mode<__half, NOIT_RESOLVE_ADAPTIVE>(ctx, A, st)
+                   : launch_mode<float, NOIT_RESOLVE_ADAPTIVE>(ctx, A, st);
+    default:
+        return f16 ? launch_mode<__half, NOIT_RESOLVE_ALL>(ctx, A, st)
+                   : launch_mode<float, NOIT_RESOLVE_ALL>(ctx, A, st);
+    }
 }
