@@ -99,6 +99,15 @@ def camera_shift_matrix(W: int, H: int) -> np.ndarray:
     return M.astype(np.float32)
 
 
+def resolve_traffic():
+    """dram bytes per launch of the plain resolve from the committed ncu capture (profiles/)."""
+    try:
+        d = json.load(open(os.path.join(ROOT, "profiles", "r01_resolve_ncu.json.txt")))
+        return int(d["dram_bytes_read"]) + int(d["dram_bytes_write"])
+    except Exception:
+        return None
+
+
 def resolve_bytes(P: int, F: int, color_bytes: int, n_images: int, depth1: bool) -> int:
     """Algorithmic bytes of the fused resolve: offsets + fragments + outputs."""
     return 4 * (P + 1) + F * (4 + color_bytes) + 16 * P * n_images + (4 * P if depth1 else 0)
@@ -300,7 +309,8 @@ def run_ours(args):
             "kernel_ms": per_kernel,
             "roofline": {"bound": "hbm", "kernel": "noit_resolve (plain fused, S1-S5)", "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                         "algorithmic_bytes": rbytes, "traffic": None},
+                         "algorithmic_bytes": rbytes, "traffic": resolve_traffic(),
+                         "traffic_source": "profiles/r01_resolve_ncu.json.txt (ncu --set full, one launch)"},
             "e2e": {"value": P * world / (e2e_ms * 1e-3) / 1e6, "unit": "Mpixels/s",
                     "what": "noit_resolve_host on the same frame, pinned host buffers",
                     "h2d_bytes_per_step": 4 * (P + 1) + 12 * F, "d2h_bytes_per_step": 16 * P,
