@@ -60,7 +60,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except OSError:
@@ -244,13 +244,15 @@ def run_ours(args):
                     pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
         if ev: ev[5].record(stream)
 
+    # clocks are sampled from the warm-up to the end of the e2e leg (the timed region alone is a
+    # few milliseconds: too short for nvidia-smi), i.e. always under this benchmark's load
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
     events = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     launches0 = ctx.launch_count
     if dist is not None:
         dist.barrier()
@@ -261,7 +263,6 @@ def run_ours(args):
     if dist is not None:
         dist.barrier()
     launches = ctx.launch_count - launches0
-    clocks = sampler.stop() if rank == 0 else None
     total_ms = events[0][0].elapsed_time(events[-1][5])
     total_ms = max_over_ranks(dist, total_ms, dev)
     per_kernel = {n: float(np.mean([e[i].elapsed_time(e[i + 1]) for e in events])) for i, n in enumerate(names)}
@@ -289,6 +290,7 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     e2e_ms = max_over_ranks(dist, e0.elapsed_time(e1) / e2e_steps, dev)
+    clocks = sampler.stop() if rank == 0 else None
     rejected = int(rp["reject_count"].item())
     hist = qt["hist"].cpu().numpy().view(np.uint32).tolist()
 

@@ -248,14 +248,12 @@ __device__ __forceinline__ void c_to_a(const float (&c)[4], float (&hi)[4], floa
     split_tf32(fmaxf(c[3], 0.f), hi[3], lo[3]);
 }
 // All 32 lanes must call this.  x = this lane's features; scratch = 32 x 12 floats of shared
-// memory private to the warp; f = tail colour of this lane's pixel.
-__device__ __forceinline__ void mlp_forward_mma(const float4* __restrict__ wp, float* scratch, int lane,
-                                                const float x[5], float f[3])
+// memory private to the warp; f = tail colour of this lane's pixel; wv = this lane's packed
+// weights, wv[v] = wp[v*32 + lane].
+__device__ __forceinline__ void mlp_forward_mma(const float4 (&wv)[NOIT_MMA_CHUNKS], float* scratch,
+                                                int lane, const float x[5], float f[3])
 {
     const int g = lane >> 2, t = lane & 3;
-    float4 wv[NOIT_MMA_CHUNKS];
-#pragma unroll
-    for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(wp + v * 32 + lane);
     auto wf = [&](int i) -> float {                           // packed value i (constant index)
         const float4& v = wv[i >> 2];
         return (i & 3) == 0 ? v.x : ((i & 3) == 1 ? v.y : ((i & 3) == 2 ? v.z : v.w));

@@ -330,9 +330,12 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     const Packed* __restrict__ g_rgba = static_cast<const Packed*>(A.rgba);
 
     // lane 0's atomic result is broadcast one tile later: its latency hides behind a tile
+    // (inline PTX: the compiler turns `if (lane == 0) atomicAdd` into a warp-aggregated atomic
+    // followed by an immediate SHFL of its result, which waits for the atomic on the spot)
     auto fetch_raw = [&]() -> uint32_t {
         uint32_t t = 0;
-        if (lane == 0) t = atomicAdd(A.tile_counter, 1u);
+        if (lane == 0)
+            asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(A.tile_counter) : "memory");
         return t;
     };
     // S9 (kMode LIST): "tile" t = entries [t*32/L, (t+1)*32/L) of the pixel list; the lists of a
@@ -601,6 +604,13 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             }
         }
         // the stage is free: start the next tile's first fill, then do this tile's MLP
+        // the MLP's packed weights (L1-resident) are requested before the fill is issued, so they
+        // are in registers when the MLP starts
+        float4 wv[NOIT_MMA_CHUNKS];
+        if (kMma) {
+#pragma unroll
+            for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(A.mlp_packed + v * 32 + lane);
+        }
         if (t_nxt < num_tiles) first_fill(no0, no1, nmixed);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
         uint32_t p = __shfl_sync(0xffffffffu, pix, (int)px_own);
@@ -619,7 +629,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 e_d1 = own.n ? own.d1 : 1.0f;
                 e_tt = own.t_tail;
             }
-            if (kMma) mlp_forward_mma(A.mlp_packed, scratch, lane, xf, f);     // all 32 lanes
+            if (kMma) mlp_forward_mma(wv, scratch, lane, xf, f);     // all 32 lanes
             else mlp_forward_packed(W, xf, f);
             if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
