@@ -6,26 +6,37 @@
 noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt, int mode,
                                        cudaStream_t st);
 
-// S7 pre-pass: G[10] of every coarse pixel whose leaf is resolved at this lod (self-contained
+// S7 pre-pass: G[10] of every coarse pixel whose leaf is resolved at that lod (self-contained
 // O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
+// One launch covers both coarse levels: blocks [0, blocks1) the half-res buffer (lod 1), the rest
+// the quarter-res buffer (lod 2).
+struct CoarseLevel {
+    int cw, ch;
+    const uint32_t* offsets;
+    const float* depth;
+    const void* rgba;
+    float* G;
+};
 template <typename ColorT>
 __global__ void __launch_bounds__(128)
-coarse_g_kernel(int cw, int ch, int r, int lod, int full_w, const uint8_t* __restrict__ cell_level,
-                uchar4 level_to_lod, const uint32_t* __restrict__ offsets,
-                const float* __restrict__ depth, const ColorT* __restrict__ rgba,
-                float* __restrict__ G)
+coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, int full_w,
+                const uint8_t* __restrict__ cell_level, uchar4 level_to_lod)
 {
-    const uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= (uint32_t)cw * (uint32_t)ch) return;
-    const int Y = q / cw, X = q - Y * cw;
+    const bool second = blockIdx.x >= blocks1;
+    const CoarseLevel lv = second ? lv2 : lv1;
+    const int lod = second ? 2 : 1, r = 1 << lod;
+    const uint32_t q = (blockIdx.x - (second ? blocks1 : 0u)) * blockDim.x + threadIdx.x;
+    if (q >= (uint32_t)lv.cw * (uint32_t)lv.ch) return;
+    const int Y = q / lv.cw, X = q - Y * lv.cw;
     const int level = cell_level[(size_t)((Y * r) >> 3) * ((full_w + 7) >> 3) + ((X * r) >> 3)] & 3;
     const uint8_t l2l[4] = {level_to_lod.x, level_to_lod.y, level_to_lod.z, level_to_lod.w};
     if (l2l[level] != lod) return;
-    const uint32_t b = __ldg(offsets + q), e = __ldg(offsets + q + 1);
+    const ColorT* __restrict__ rgba = static_cast<const ColorT*>(lv.rgba);
+    const uint32_t b = __ldg(lv.offsets + q), e = __ldg(lv.offsets + q + 1);
     PixelState<false> s;
     s.init();
-    for (uint32_t j = b; j < e; ++j) s.push(__ldg(depth + j), load_rgba(rgba, j), j);
-    float* g = G + 10 * (size_t)q;
+    for (uint32_t j = b; j < e; ++j) s.push(__ldg(lv.depth + j), load_rgba(rgba, j), j);
+    float* g = lv.G + 10 * (size_t)q;
     g[0] = s.c2.w * s.c2.x; g[1] = s.c2.w * s.c2.y; g[2] = s.c2.w * s.c2.z; g[3] = s.c2.w;
     g[4] = s.acc_r; g[5] = s.acc_g; g[6] = s.acc_b; g[7] = s.a_tail; g[8] = s.t_tail;
     g[9] = (float)(e - b);
@@ -93,6 +104,9 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
         memcpy(A.level_to_lod, d->level_to_lod, 4);
         const uchar4 l2l = make_uchar4(d->level_to_lod[0], d->level_to_lod[1], d->level_to_lod[2],
                                        d->level_to_lod[3]);
+        CoarseLevel lv[2];
+        memset(lv, 0, sizeof lv);
+        uint32_t blocks[2] = {0, 0};
         for (int lod = 1; lod <= 2; ++lod) {
             bool used = false;
             for (int l = 0; l < 4; ++l) used |= d->level_to_lod[l] == lod;
@@ -112,15 +126,17 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
             A.coarse_g[lod - 1] = ctx->d_coarse_g[lod - 1];
             A.coarse_w[lod - 1] = cb->width;
             A.coarse_h[lod - 1] = cb->height;
-            const uint32_t blocks = (uint32_t)((cp + 127) / 128);
+            lv[lod - 1] = CoarseLevel{cb->width, cb->height, cb->offsets, cb->depth, cb->rgba,
+                                      ctx->d_coarse_g[lod - 1]};
+            blocks[lod - 1] = (uint32_t)((cp + 127) / 128);
+        }
+        if (blocks[0] + blocks[1]) {
             if (fmt == NOIT_RGBA_F16)
-                coarse_g_kernel<__half><<<blocks, 128, 0, st>>>(
-                    cb->width, cb->height, 1 << lod, lod, A.W, d->cell_level, l2l, cb->offsets,
-                    cb->depth, (const __half*)cb->rgba, ctx->d_coarse_g[lod - 1]);
+                coarse_g_kernel<__half><<<blocks[0] + blocks[1], 128, 0, st>>>(
+                    lv[0], lv[1], blocks[0], A.W, d->cell_level, l2l);
             else
-                coarse_g_kernel<float><<<blocks, 128, 0, st>>>(
-                    cb->width, cb->height, 1 << lod, lod, A.W, d->cell_level, l2l, cb->offsets,
-                    cb->depth, (const float*)cb->rgba, ctx->d_coarse_g[lod - 1]);
+                coarse_g_kernel<float><<<blocks[0] + blocks[1], 128, 0, st>>>(
+                    lv[0], lv[1], blocks[0], A.W, d->cell_level, l2l);
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
         }

@@ -459,12 +459,10 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         left -= 1u;
         uint32_t no0 = 0, no1 = 0, npix = 0;
         int nlod = 0, nlevel = 3;
-        bool nmixed = false;
         if (t_nxt < num_tiles) {                         // lands while this tile runs
             npix = lane_pixel(t_nxt);
             load_offsets(npix, no0, no1);
             nlod = lane_lod(npix, nlevel);
-            nmixed = __any_sync(0xffffffffu, nlod > 0);
         }
 
         Owned<ColorT> own;
@@ -611,6 +609,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 #pragma unroll
             for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(A.mlp_packed + v * 32 + lane);
         }
+        // (the vote is taken here, not where the level was requested: it would wait for the load)
+        const bool nmixed = kMode == NOIT_RESOLVE_ADAPTIVE && __any_sync(0xffffffffu, nlod > 0);
         if (t_nxt < num_tiles) first_fill(no0, no1, nmixed);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
         uint32_t p = __shfl_sync(0xffffffffu, pix, (int)px_own);
