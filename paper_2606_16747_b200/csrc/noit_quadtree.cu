@@ -56,8 +56,7 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
                 uint32_t* __restrict__ hist)
 {
     __shared__ Moments cell[64];          // 8x8 cells, index cy*8 + cx
-    __shared__ uint8_t split[21];         // node split flags: 0 root, 1..4 level 1, 5..20 level 2
-    __shared__ uint8_t lvl[64];
+    __shared__ Moments node2[16];         // level-2 nodes (16x16 pixels), index 4c + g
     const int Tx = (W + 63) >> 6;
     const int tile = blockIdx.x, tx = tile % Tx, ty = tile / Tx;
     const int X = tx << 6, Y = ty << 6;
@@ -104,80 +103,107 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
                 cell[warp * 8 + i] = m;
             }
         }
-        __syncthreads();
-        if (threadIdx.x < 21) {
-            // node -> rectangle of cells: level 0: 8x8 cells, level 1: 4x4, level 2: 2x2
-            int cx0, cy0, span;
-            const int t = threadIdx.x;
-            if (t == 0) { cx0 = 0; cy0 = 0; span = 8; }
-            else if (t < 5) { const int c = t - 1; cx0 = 4 * (c & 1); cy0 = 4 * (c >> 1); span = 4; }
-            else {
-                const int c = (t - 5) >> 2, g = (t - 5) & 3;
-                cx0 = 4 * (c & 1) + 2 * (g & 1); cy0 = 4 * (c >> 1) + 2 * (g >> 1); span = 2;
-            }
-            Moments m = {0, {0, 0, 0}, {0, 0, 0}};
-            for (int v = 0; v < span; ++v)
-                for (int u = 0; u < span; ++u) {
+    }
+    __syncthreads();
+    if (warp != 0) return;
+    // ---- warp 0: node statistics bottom-up, split tests, mask, cell levels, histogram.
+    // Lane t < 21 owns node t: 0 root, 1..4 level 1 (c = t-1), 5..20 level 2 (c = (t-5)>>2,
+    // g = (t-5)&3) -- the same numbering as the mask bits.
+    bool flag = false;
+    if (metric == NOIT_QT_VARIANCE) {
+        Moments m = {0, {0, 0, 0}, {0, 0, 0}};
+        if (lane >= 5 && lane < 21) {                    // level 2: 2x2 cells
+            const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+            const int cx0 = 4 * (c & 1) + 2 * (g & 1), cy0 = 4 * (c >> 1) + 2 * (g >> 1);
+#pragma unroll
+            for (int v = 0; v < 2; ++v)
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
                     const Moments& q = cell[(cy0 + v) * 8 + cx0 + u];
                     m.n += q.n;
-                    for (int c = 0; c < 3; ++c) { m.s1[c] += q.s1[c]; m.s2[c] += q.s2[c]; }
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { m.s1[k] += q.s1[k]; m.s2[k] += q.s2[k]; }
                 }
-            split[t] = variance_splits(m, var_thr);
+            node2[lane - 5] = m;
         }
-    } else {
-        if (threadIdx.x < 21) {
-            int x0, y0, side;
-            const int t = threadIdx.x;
-            if (t == 0) { x0 = X; y0 = Y; side = 64; }
-            else if (t < 5) { const int c = t - 1; x0 = X + 32 * (c & 1); y0 = Y + 32 * (c >> 1); side = 32; }
-            else {
-                const int c = (t - 5) >> 2, g = (t - 5) & 3;
-                x0 = X + 32 * (c & 1) + 16 * (g & 1); y0 = Y + 32 * (c >> 1) + 16 * (g >> 1); side = 16;
+        __syncwarp();
+        if (lane >= 1 && lane < 5) {                     // level 1: its 4 level-2 children
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                const Moments& q = node2[4 * (lane - 1) + g];
+                m.n += q.n;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { m.s1[k] += q.s1[k]; m.s2[k] += q.s2[k]; }
             }
-            split[t] = corner_splits(image, W, H, x0, y0, side, corner_thr);
         }
+        if (lane == 0) {                                 // root: all 16 level-2 nodes
+            for (int g = 0; g < 16; ++g) {
+                const Moments& q = node2[g];
+                m.n += q.n;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { m.s1[k] += q.s1[k]; m.s2[k] += q.s2[k]; }
+            }
+        }
+        flag = lane < 21 && variance_splits(m, var_thr);
+    } else if (lane < 21) {
+        int x0 = X, y0 = Y, side = 64;
+        if (lane >= 5) {
+            const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+            x0 = X + 32 * (c & 1) + 16 * (g & 1); y0 = Y + 32 * (c >> 1) + 16 * (g >> 1); side = 16;
+        } else if (lane >= 1) {
+            const int c = lane - 1;
+            x0 = X + 32 * (c & 1); y0 = Y + 32 * (c >> 1); side = 32;
+        }
+        flag = corner_splits(image, W, H, x0, y0, side, corner_thr);
     }
-    __syncthreads();
-    // top-down: a node's flag counts only if its parent split.  Thread c (8x8 cell c).
-    if (threadIdx.x < 64) {
-        const int cx = threadIdx.x & 7, cy = threadIdx.x >> 3;
+    // top-down: a node's flag counts only if its parent split
+    const uint32_t F = __ballot_sync(0xffffffffu, flag);
+    uint32_t mask = 0;
+    if (F & 1u) {
+        mask = 1u;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if ((F >> (1 + c)) & 1u) mask |= (1u << (1 + c)) | (F & (0xFu << (5 + 4 * c)));
+    }
+    auto level_of_cell = [&](int cx, int cy) -> int {
         const int c = (cx >> 2) + 2 * (cy >> 2), g = ((cx >> 1) & 1) + 2 * ((cy >> 1) & 1);
-        int level = 0;
-        if (split[0]) {
-            level = 1;
-            if (split[1 + c]) level = split[5 + 4 * c + g] ? 3 : 2;
-        }
-        lvl[threadIdx.x] = (uint8_t)level;
+        if (!(mask & 1u)) return 0;
+        if (!((mask >> (1 + c)) & 1u)) return 1;
+        return ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
+    };
+    const int cells_w = (W + 7) >> 3, cells_h = (H + 7) >> 3;
+    uint32_t h3 = 0;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {                        // 64 cells, 2 per lane
+        const int idx = lane + 32 * k, cx = idx & 7, cy = idx >> 3;
+        const int level = level_of_cell(cx, cy);
         const int gx = (X >> 3) + cx, gy = (Y >> 3) + cy;
-        if (cell_level && gx < ((W + 7) >> 3) && gy < ((H + 7) >> 3))
-            cell_level[(size_t)gy * ((W + 7) >> 3) + gx] = (uint8_t)level;
+        const bool in_image = gx < cells_w && gy < cells_h;
+        if (cell_level && in_image) cell_level[(size_t)gy * cells_w + gx] = (uint8_t)level;
+        h3 += __popc(__ballot_sync(0xffffffffu, in_image && level == 3));
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t mask = 0;
-        if (split[0]) {
-            mask |= 1u;
-            for (int c = 0; c < 4; ++c)
-                if (split[1 + c]) {
-                    mask |= 1u << (1 + c);
-                    for (int g = 0; g < 4; ++g)
-                        if (split[5 + 4 * c + g]) mask |= 1u << (5 + 4 * c + g);
-                }
-        }
-        if (tile_mask) tile_mask[tile] = mask;
-        if (hist) {
-            // leaves with >= 1 in-image pixel: a leaf at level l is counted at its first cell
-            uint32_t h[4] = {0, 0, 0, 0};
-            for (int level = 0; level < 4; ++level) {
-                const int side = 64 >> level, per = 1 << level, cs = side >> 3;
-                for (int ny = 0; ny < per; ++ny)
-                    for (int nx = 0; nx < per; ++nx) {
-                        if (X + nx * side >= W || Y + ny * side >= H) continue;
-                        if (lvl[(ny * cs) * 8 + nx * cs] == level) h[level] += 1;
-                    }
+    if (tile_mask && lane == 0) tile_mask[tile] = mask;
+    if (hist) {
+        // leaves with >= 1 in-image pixel: the node at level l whose first cell has level l
+        bool leaf = false;
+        int lv = 0;
+        if (lane < 21) {
+            int cx = 0, cy = 0;
+            if (lane >= 5) {
+                const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+                cx = 4 * (c & 1) + 2 * (g & 1); cy = 4 * (c >> 1) + 2 * (g >> 1); lv = 2;
+            } else if (lane >= 1) {
+                cx = 4 * ((lane - 1) & 1); cy = 4 * ((lane - 1) >> 1); lv = 1;
             }
-            for (int level = 0; level < 4; ++level)
-                if (h[level]) atomicAdd(hist + level, h[level]);
+            leaf = X + 8 * cx < W && Y + 8 * cy < H && level_of_cell(cx, cy) == lv;
+        }
+        const uint32_t Lf = __ballot_sync(0xffffffffu, leaf);
+        if (lane == 0) {
+            const uint32_t h0 = Lf & 1u, h1 = __popc(Lf & 0x1Eu), h2 = __popc(Lf & 0x1FFFE0u);
+            if (h0) atomicAdd(hist + 0, h0);
+            if (h1) atomicAdd(hist + 1, h1);
+            if (h2) atomicAdd(hist + 2, h2);
+            if (h3) atomicAdd(hist + 3, h3);
         }
     }
 }

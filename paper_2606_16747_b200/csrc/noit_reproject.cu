@@ -10,6 +10,7 @@ struct ReprojArgs {
     int32_t W, H;
     float M[16];
     float thr;
+    float inv_w, inv_h;            // 1.0f / W, 1.0f / H (IEEE fp32, formed once on the host)
     float bg[3];
     const float* prev_trans; const float* prev_depth; const float* cur_depth;
     float* out_trans; float* out_depth; float* out_final;
@@ -26,9 +27,8 @@ reproject_kernel(const __grid_constant__ ReprojArgs A)
     if (inside) {
         p = (uint32_t)y * (uint32_t)A.W + (uint32_t)x;
         const float fW = (float)A.W, fH = (float)A.H;
-        const float inv_w = __fdiv_rn(1.0f, fW), inv_h = __fdiv_rn(1.0f, fH);
-        const float xn = __fmaf_rn(__fmul_rn(2.0f, __fadd_rn((float)x, 0.5f)), inv_w, -1.0f);
-        const float yn = __fmaf_rn(__fmul_rn(2.0f, __fadd_rn((float)y, 0.5f)), inv_h, -1.0f);
+        const float xn = __fmaf_rn(__fmul_rn(2.0f, __fadd_rn((float)x, 0.5f)), A.inv_w, -1.0f);
+        const float yn = __fmaf_rn(__fmul_rn(2.0f, __fadd_rn((float)y, 0.5f)), A.inv_h, -1.0f);
         const float d = __ldcs(A.cur_depth + p);
         float c[4];
 #pragma unroll
@@ -86,6 +86,8 @@ extern "C" noit_status noit_reproject(noit_ctx* ctx, const noit_reproject_desc* 
     A.W = d->width; A.H = d->height;
     memcpy(A.M, d->M, sizeof A.M);
     A.thr = d->depth_threshold;
+    A.inv_w = 1.0f / (float)d->width;      // same correctly rounded fp32 quotient as O8's 1.0f/W
+    A.inv_h = 1.0f / (float)d->height;
     memcpy(A.bg, d->background, sizeof A.bg);
     A.prev_trans = d->prev_trans; A.prev_depth = d->prev_depth; A.cur_depth = d->cur_depth;
     A.out_trans = d->out_trans; A.out_depth = d->out_depth; A.out_final = d->out_final;
