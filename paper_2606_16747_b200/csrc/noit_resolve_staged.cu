@@ -36,7 +36,6 @@ namespace {
 constexpr uint32_t kCap = 1000;          // fragments per warp stage (12000 B with fp16 colour: 16 warps/SM)
 constexpr uint32_t kScratchFloats = 32 * 12;   // per warp: feature / output transpose of the MMA MLP
 constexpr int kWarpsPerCta = 4;
-constexpr uint32_t kTileBatch = 1;       // tiles per atomic (4 measured slower: 204 vs 168 us, heavy tiles cluster)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
 {
@@ -255,9 +254,9 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
         Top2 s;
         s.d1 = s.d2 = __int_as_float(0x7f800000);
         s.i1 = s.i2 = NOIT_ABSENT;
-        // latency-bound (scattered lists): four loads in flight per lane, and the colours are
+        // latency-bound (scattered lists): eight loads in flight per lane, and the colours are
         // pulled into L2 while the depths are scanned
-#pragma unroll 4
+#pragma unroll 8
         for (uint32_t j = b + q; j < e; j += L) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(rgba + j));
             top2_push(s, __ldg(depth + j), j);
@@ -267,7 +266,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
             top2_merge(s, __shfl_xor_sync(0xffffffffu, s.d1, m), __shfl_xor_sync(0xffffffffu, s.i1, m),
                        __shfl_xor_sync(0xffffffffu, s.d2, m), __shfl_xor_sync(0xffffffffu, s.i2, m));
         float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f;
-#pragma unroll 4
+#pragma unroll 8
         for (uint32_t j = b + q; j < e; j += L) {
             typename Color<ColorT>::Packed raw = __ldg(rgba + j);
             if (j == s.i1 || j == s.i2) raw = Color<ColorT>::zero_alpha_reg(raw);
@@ -332,10 +331,15 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // lane 0's atomic result is broadcast one tile later: its latency hides behind a tile
     // (inline PTX: the compiler turns `if (lane == 0) atomicAdd` into a warp-aggregated atomic
     // followed by an immediate SHFL of its result, which waits for the atomic on the spot)
+    // The first three tiles of a warp are static (warp id + k * warps): no atomic round trips at
+    // start-up; the counter hands out the tiles after those.
+    const uint32_t n_warps = gridDim.x * kWarpsPerCta, warp_id = blockIdx.x * kWarpsPerCta + warp;
     auto fetch_raw = [&]() -> uint32_t {
         uint32_t t = 0;
-        if (lane == 0)
+        if (lane == 0) {
             asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(A.tile_counter) : "memory");
+            t += 3u * n_warps;
+        }
         return t;
     };
     // S9 (kMode LIST): "tile" t = entries [t*32/L, (t+1)*32/L) of the pixel list; the lists of a
@@ -433,11 +437,10 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         }
     };
 
-    // tiles are taken in batches of kTileBatch consecutive tiles per atomic: same-address
-    // atomics are serialised by the L2, one per tile would cap the kernel
-    uint32_t t_cur = __shfl_sync(0xffffffffu, fetch_raw(), 0) * kTileBatch;
-    uint32_t raw_nxt = fetch_raw(), raw_nn = fetch_raw();   // two atomics in flight
-    uint32_t left = kTileBatch - 1;                      // tiles of the current batch after t_cur
+    // one tile per atomic (4 consecutive tiles per atomic measured slower, 204 vs 168 us: heavy
+    // tiles cluster and the load imbalance costs more than the atomics)
+    uint32_t t_cur = warp_id;
+    uint32_t raw_nxt = warp_id + n_warps, raw_nn = warp_id + 2u * n_warps;   // then two atomics in flight
     uint32_t o0 = 0, o1 = 0, pix = 0;
     int lod = 0, level = 3;
     bool mixed = false;                                  // S7: the tile has pixels with lod > 0
@@ -449,14 +452,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         first_fill(o0, o1, mixed);
     }
     while (t_cur < num_tiles) {
-        uint32_t t_nxt = t_cur + 1u;
-        if (left == 0) {
-            t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0) * kTileBatch;
-            raw_nxt = raw_nn;
-            raw_nn = fetch_raw();
-            left = kTileBatch;
-        }
-        left -= 1u;
+        const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
+        raw_nxt = raw_nn;
+        raw_nn = fetch_raw();
         uint32_t no0 = 0, no1 = 0, npix = 0;
         int nlod = 0, nlevel = 3;
         if (t_nxt < num_tiles) {                         // lands while this tile runs
@@ -678,8 +676,11 @@ static noit_status launch_mode(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t
     // bf16-rounded weights are exact in TF32: the MLP runs on the tensor cores (two-pass split
     // of the activations, fp32-class accuracy); fp32 weights keep the FFMA2 form.
     const bool mma = ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp != nullptr;
-    return mma ? launch_staged<ColorT, 4, true, kMode>(ctx, A, st)
-               : launch_staged<ColorT, 4, false, kMode>(ctx, A, st);
+    // lanes per pixel: 4 for frames; 8 for the pixel list (scattered lists are latency-bound:
+    // shorter per-lane chains, 4-pixel tiles keep every warp of the machine busy)
+    constexpr int L = kMode == NOIT_RESOLVE_LIST ? 8 : 4;
+    return mma ? launch_staged<ColorT, L, true, kMode>(ctx, A, st)
+               : launch_staged<ColorT, L, false, kMode>(ctx, A, st);
 }
 
 noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int color_fmt, int mode,
