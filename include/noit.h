@@ -17,7 +17,9 @@
  *  - Device-side preconditions are documented, not checked: offsets non-decreasing with
  *    offsets[P] == num_fragments; depth finite; alpha in [0,1]; inputs and outputs do not alias
  *    (except noit_reproject's cur_depth == prev_depth, which is allowed).
- *  - A context is not thread-safe; distinct contexts are independent.
+ *  - A context is not thread-safe; distinct contexts are independent.  Calls on ONE context must
+ *    be stream-ordered with respect to each other (same stream, or ordered by events): the
+ *    context owns small device scratch (work counters, S7 intermediates) that launches share.
  *  - There is no CPU fallback and no other backend.
  *
  * Fragment buffer layout (S:8(a) S0; stands in for the paper's three raster passes P:55):

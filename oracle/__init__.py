@@ -145,6 +145,22 @@ def quadtree(image: np.ndarray, width: int, height: int, metric: int = 0,
     return out
 
 
+def quadtree_balance(tile_mask: np.ndarray, width: int, height: int, iterations: int = 2,
+                     delta2: float = 2.2, delta3: float = 3.0) -> dict:
+    """O10: 2:1 tile balance by Jacobi relaxation + histogram + demand index and Eq. 2 scales."""
+    Tx, Ty = (width + 63) // 64, (height + 63) // 64
+    cx, cy = (width + 7) // 8, (height + 7) // 8
+    out = dict(tile_mask=_chk(np.array(tile_mask, np.uint32), np.uint32, Tx * Ty),
+               tile_level=np.zeros(Tx * Ty, np.uint8), cell_level=np.zeros(cx * cy, np.uint8),
+               hist=np.zeros(4, np.uint32), scales=np.zeros(3, np.float32))
+    rc = lib().oracle_quadtree_balance(C.c_int32(width), C.c_int32(height), C.c_int32(iterations),
+                                       C.c_float(delta2), C.c_float(delta3), _p(out["tile_mask"]),
+                                       _p(out["tile_level"]), _p(out["cell_level"]), _p(out["hist"]),
+                                       _p(out["scales"]))
+    assert rc == 0
+    return out
+
+
 def reproject(width, height, M, depth_threshold, background, prev_trans, prev_depth, cur_depth,
               out_trans=None, out_depth=None, out_final=None) -> dict:
     P = width * height

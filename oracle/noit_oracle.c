@@ -519,6 +519,89 @@ int32_t oracle_quadtree(const float *image, int32_t width, int32_t height, int32
 }
 
 /* ---------------------------------------------------------------------------------------- */
+/* O10 quadtree consistency + demand index.          */
+/* "neighboring tiles may differ by at most one refinement level ... since refinement levels    */
+/* are limited to {0,1,2,3}, two relaxation iterations (k=2) are sufficient".  Reading   */
+/* A25: the level of a base tile is the depth of its subtree (0 = unsplit .. 3 = a  */
+/* grandchild split); one relaxation iteration is the Jacobi step                               */
+/*     L_i <- max(L_i, max over the 4 edge neighbours j of L_j - 1)                             */
+/* evaluated for all tiles from the PREVIOUS iteration's levels; a tile whose level rises to L  */
+/* is refined uniformly to depth L (every node above depth L splits), which keeps the mask      */
+/* valid (child bit => parent bit).  Then cell levels and the histogram of occupied leaves are  */
+/* recomputed, w = sum l N_l / sum N_l and s_p = clamp(2^(w - delta_p), 0.25, 1) (Eq. 2  */
+/* P:80) with delta_2 = 2.2, delta_3 = 3.0 are formed in double.                                */
+static int mask_depth(uint32_t mask)
+{
+    if (!(mask & 1u)) return 0;
+    if (!(mask & 0x1Eu)) return 1;
+    if (!(mask & 0x1FFFE0u)) return 2;
+    return 3;
+}
+
+int32_t oracle_quadtree_balance(int32_t width, int32_t height, int32_t iterations, float delta2,
+                                float delta3, uint32_t *tile_mask, uint8_t *tile_level,
+                                uint8_t *cell_level, uint32_t *hist, float *scales)
+{
+    int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
+    int cells_x = (width + 7) / 8, cells_y = (height + 7) / 8;
+    int n = Tx * Ty;
+    int *cur = (int *)malloc(sizeof(int) * (size_t)n), *nxt = (int *)malloc(sizeof(int) * (size_t)n);
+    if (!cur || !nxt) { free(cur); free(nxt); return 1; }
+    for (int i = 0; i < n; ++i) cur[i] = mask_depth(tile_mask[i]);
+    for (int it = 0; it < iterations; ++it) {
+        for (int ty = 0; ty < Ty; ++ty)
+            for (int tx = 0; tx < Tx; ++tx) {
+                int best = cur[ty * Tx + tx];
+                if (tx > 0 && cur[ty * Tx + tx - 1] - 1 > best) best = cur[ty * Tx + tx - 1] - 1;
+                if (tx + 1 < Tx && cur[ty * Tx + tx + 1] - 1 > best) best = cur[ty * Tx + tx + 1] - 1;
+                if (ty > 0 && cur[(ty - 1) * Tx + tx] - 1 > best) best = cur[(ty - 1) * Tx + tx] - 1;
+                if (ty + 1 < Ty && cur[(ty + 1) * Tx + tx] - 1 > best) best = cur[(ty + 1) * Tx + tx] - 1;
+                nxt[ty * Tx + tx] = best;
+            }
+        int *t = cur; cur = nxt; nxt = t;
+    }
+    uint64_t h[4] = {0, 0, 0, 0};
+    for (int ty = 0; ty < Ty; ++ty)
+        for (int tx = 0; tx < Tx; ++tx) {
+            int i = ty * Tx + tx, L = cur[i], X = tx * 64, Y = ty * 64;
+            uint32_t mask = tile_mask[i];
+            if (L >= 1) mask |= 1u;                      /* every node above depth L splits */
+            if (L >= 2) mask |= 0x1Eu;
+            if (L >= 3) mask |= 0x1FFFE0u;
+            tile_mask[i] = mask;
+            if (tile_level) tile_level[i] = (uint8_t)L;
+            for (int v = 0; v < 8; ++v)
+                for (int u = 0; u < 8; ++u) {
+                    int c = (u >> 2) + 2 * (v >> 2), g = ((u >> 1) & 1) + 2 * ((v >> 1) & 1);
+                    int level = 0;
+                    if (mask & 1u) {
+                        level = 1;
+                        if ((mask >> (1 + c)) & 1u) level = ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
+                    }
+                    int cxg = X / 8 + u, cyg = Y / 8 + v;
+                    if (cxg >= cells_x || cyg >= cells_y) continue;
+                    if (cell_level) cell_level[cyg * cells_x + cxg] = (uint8_t)level;
+                    /* a leaf is counted at its first (top-left) cell, which is in the image  */
+                    /* whenever the leaf holds an in-image pixel                              */
+                    int span = 8 >> level;              /* leaf side in cells */
+                    if (u % span == 0 && v % span == 0) h[level] += 1;
+                }
+        }
+    if (hist) for (int k = 0; k < 4; ++k) hist[k] = (uint32_t)h[k];
+    if (scales) {
+        double num = 0.0, den = 0.0;
+        for (int k = 0; k < 4; ++k) { num += (double)k * (double)h[k]; den += (double)h[k]; }
+        double w = den > 0.0 ? num / den : 0.0;
+        double s2 = pow(2.0, w - (double)delta2), s3 = pow(2.0, w - (double)delta3);
+        s2 = s2 < 0.25 ? 0.25 : (s2 > 1.0 ? 1.0 : s2);
+        s3 = s3 < 0.25 ? 0.25 : (s3 > 1.0 ? 1.0 : s3);
+        scales[0] = (float)w; scales[1] = (float)s2; scales[2] = (float)s3;
+    }
+    free(cur); free(nxt);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
 /* O8 reprojection ("reprojecting pixels using the nearest available depth and the       */
 /* previous view-projection matrix"; P:53 first-fragment depth reused).  All fp32, operations  */
 /* exactly in this order; every fmaf is a real fused op; nothing else is contracted.           */

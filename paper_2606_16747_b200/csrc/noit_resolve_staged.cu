@@ -1,6 +1,8 @@
 // noit_resolve_staged.cu -- the plain fused resolve (S1-S5, Eq. 4) of a whole frame:
 // persistent warps, fragment ranges staged into shared memory by 1-D TMA bulk copies
-// (cp.async.bulk + mbarrier), two passes over the staged lists, MLP with packed FFMA2.
+// (cp.async.bulk + mbarrier), two passes over the staged lists, MLP on the tensor cores
+// (mma.sync TF32 with a two-pass activation split) or with packed FFMA2 (fp32 weights).
+// One kernel, three modes: whole frame (S1-S5), adaptive frame (S7), pixel list (S9).
 //
 // Why this shape (ncu evidence in profiles/r01_*): a thread-per-pixel kernel that reads its
 // list straight from global memory is bound by L1 data-stage wavefronts (every lane of a load
@@ -25,8 +27,9 @@
 //     group with round q's merged top-2 (log2(L) exchange steps, L-1 merges, instead of L full
 //     butterflies); then for colours only, in chunks of rounds, pass 2, and one transposed
 //     butterfly of the five sums;
-//   * every lane then owns one pixel: features, MLP (FFMA2: two output neurons per
-//     instruction, same summation order as the scalar form), composite, 128-bit stores.
+//   * every lane then owns one pixel: features, MLP (noit_internal.cuh: mlp_forward_mma /
+//     mlp_forward_packed), composite, 128-bit stores.  The next tile's first fill is issued
+//     before the MLP, which hides its latency.
 // Tiles are handed out by an atomic counter (fragment counts vary 0..128 per pixel) whose result
 // is broadcast one tile later, and which the last warp to finish resets (no memset per launch).
 #include "noit_resolve_common.cuh"

@@ -614,3 +614,123 @@ def test_fallback_covers_every_pixel_once(cfg1_scene):
     oracle.resolve(fb, w, BG, pixel_list=rp2["reject_list"], out=out2)
     for k in ("trans", "final", "depth1"):
         assert np.array_equal(out2[k], plain[k])
+
+
+# -------------------------------------------------------------------------------------------
+# O10: quadtree consistency (2:1 balance by Jacobi relaxation), histogram, demand index, Eq. 2
+# ("two relaxation iterations (k=2) are sufficient", :78 w-bar, :80-85 Eq. 2)
+# -------------------------------------------------------------------------------------------
+FULL = {0: 0x0, 1: 0x1, 2: 0x1F, 3: 0x1FFFFF}
+
+
+def _depth(mask):
+    return 0 if not mask & 1 else (1 if not mask & 0x1E else (2 if not mask & 0x1FFFE0 else 3))
+
+
+def _random_valid_masks(rng, n):
+    out = np.zeros(n, np.uint32)
+    for i in range(n):
+        m = 0
+        if rng.random() < 0.5:
+            m |= 1
+            for c in range(4):
+                if rng.random() < 0.5:
+                    m |= 1 << (1 + c)
+                    for g in range(4):
+                        if rng.random() < 0.4:
+                            m |= 1 << (5 + 4 * c + g)
+        out[i] = m
+    return out
+
+
+def test_balance_single_deep_tile_gives_diamond():
+    Tx, Ty = 9, 7
+    m = np.zeros(Tx * Ty, np.uint32)
+    m[3 * Tx + 4] = FULL[3]
+    r = oracle.quadtree_balance(m, Tx * 64, Ty * 64)
+    yy, xx = np.mgrid[0:Ty, 0:Tx]
+    want = np.maximum(0, 3 - (np.abs(yy - 3) + np.abs(xx - 4)))          # closed form
+    assert np.array_equal(r["tile_level"].reshape(Ty, Tx), want)
+    assert np.array_equal(r["tile_mask"].reshape(Ty, Tx), np.vectorize(FULL.get)(want))
+    # one iteration is NOT enough (3 | 2 | 0), the paper's k = 2 is
+    r1 = oracle.quadtree_balance(m, Tx * 64, Ty * 64, iterations=1)
+    assert r1["tile_level"].reshape(Ty, Tx)[3, 6] == 0 and r1["tile_level"].reshape(Ty, Tx)[3, 5] == 2
+
+
+@pytest.mark.parametrize("seed,Tx,Ty,W,H", [(0, 12, 9, 12 * 64, 9 * 64), (1, 30, 17, 1920, 1080),
+                                            (2, 1, 1, 40, 40), (3, 5, 1, 300, 50)])
+def test_balance_properties_and_maxplus_closed_form(seed, Tx, Ty, W, H):
+    rng = np.random.default_rng(seed)
+    m = _random_valid_masks(rng, Tx * Ty)
+    r = oracle.quadtree_balance(m, W, H)
+    L0 = np.array([_depth(int(x)) for x in m]).reshape(Ty, Tx)
+    L = r["tile_level"].reshape(Ty, Tx).astype(int)
+    # k Jacobi steps of L <- max(L, max_nbr L - 1) == max-plus convolution with the Manhattan
+    # diamond of radius k: brute force over all tile pairs
+    want = L0.copy()
+    for y in range(Ty):
+        for x in range(Tx):
+            for v in range(Ty):
+                for u in range(Tx):
+                    d = abs(y - v) + abs(x - u)
+                    if d <= 2:
+                        want[y, x] = max(want[y, x], L0[v, u] - d)
+    assert np.array_equal(L, want)
+    assert np.all(np.abs(np.diff(L, axis=0)) <= 1) and np.all(np.abs(np.diff(L, axis=1)) <= 1)
+    # masks: original bits kept, refined uniformly to the new depth, child bit => parent bit
+    for i, (a, b) in enumerate(zip(m, r["tile_mask"])):
+        a, b = int(a), int(b)
+        assert b == a | FULL[int(L.reshape(-1)[i])]
+        for c in range(4):
+            if b >> (1 + c) & 1:
+                assert b & 1
+            for g in range(4):
+                if b >> (5 + 4 * c + g) & 1:
+                    assert b >> (1 + c) & 1
+    # balancing a balanced forest changes nothing
+    r2 = oracle.quadtree_balance(r["tile_mask"], W, H)
+    assert np.array_equal(r2["tile_mask"], r["tile_mask"]) and np.array_equal(r2["hist"], r["hist"])
+    # cell levels and histogram against a direct recount from the masks
+    cw, chh = (W + 7) // 8, (H + 7) // 8
+    hist = np.zeros(4, np.int64)
+    for ty in range(Ty):
+        for tx in range(Tx):
+            b = int(r["tile_mask"][ty * Tx + tx])
+            for level in range(4):
+                side, per = 64 >> level, 1 << level
+                for ny in range(per):
+                    for nx in range(per):
+                        x0, y0 = tx * 64 + nx * side, ty * 64 + ny * side
+                        if x0 >= W or y0 >= H:
+                            continue
+                        # the node exists iff all its ancestors split; it is a leaf iff it does not
+                        c = (nx * side // 32) + 2 * (ny * side // 32)
+                        g = ((nx * side // 16) & 1) + 2 * ((ny * side // 16) & 1)
+                        anc = [True, bool(b & 1), bool(b & 1 and b >> (1 + c) & 1),
+                               bool(b & 1 and b >> (1 + c) & 1 and b >> (5 + 4 * c + g) & 1)]
+                        own = [bool(b & 1), bool(b >> (1 + c) & 1), bool(b >> (5 + 4 * c + g) & 1), False]
+                        if anc[level] and not own[level]:
+                            hist[level] += 1
+                            for cy in range(y0 // 8, min((y0 + side + 7) // 8, chh)):
+                                for cx in range(x0 // 8, min((x0 + side + 7) // 8, cw)):
+                                    if cx * 8 < min(x0 + side, W) and cy * 8 < min(y0 + side, H):
+                                        assert r["cell_level"][cy * cw + cx] == level
+    assert np.array_equal(r["hist"].astype(np.int64), hist)
+
+
+def test_demand_index_and_eq2_fixed_points():
+    """s_2 = 1 at w = 2.2, s_3 = 1 at w = 3.0, both floored at 0.25."""
+    # 16 tiles refined to depth 2 (256 leaves at level 2) + 1 tile fully refined (64 at level 3):
+    # w = (2*256 + 3*64) / 320 = 2.2 exactly
+    m = np.array([FULL[2]] * 16 + [FULL[3]], np.uint32)
+    r = oracle.quadtree_balance(m, 17 * 64, 64)
+    assert r["hist"].tolist() == [0, 0, 256, 64]
+    assert abs(r["scales"][0] - 2.2) < 1e-6 and abs(r["scales"][1] - 1.0) < 1e-6
+    assert abs(r["scales"][2] - 2.0 ** (2.2 - 3.0)) < 1e-6
+    r = oracle.quadtree_balance(np.full(6, FULL[3], np.uint32), 3 * 64, 2 * 64)       # w = 3
+    assert r["scales"].tolist() == [3.0, 1.0, 1.0]
+    r = oracle.quadtree_balance(np.zeros(6, np.uint32), 3 * 64, 2 * 64)               # w = 0: floor
+    assert r["scales"].tolist() == [0.0, 0.25, 0.25]
+    r = oracle.quadtree_balance(np.full(6, FULL[2], np.uint32), 3 * 64, 2 * 64)       # w = 2
+    assert r["scales"][0] == 2.0 and r["scales"][2] == 0.5
+    assert abs(r["scales"][1] - 0.8705505632961241) < 1e-6                            # 2^-0.2
