@@ -158,6 +158,24 @@ noit_status noit_quadtree(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t 
                           int32_t height, const noit_qt_params* params, uint32_t* tile_mask,
                           uint8_t* cell_level, uint32_t* level_hist, void* stream);
 
+/* ---- NEXT-1: quadtree consistency + demand index (O10, reading A25).
+ * "neighboring tiles may differ by at most one refinement level ... two relaxation iterations
+ * (k=2) are sufficient": the level of a base tile is the depth of its subtree (0 = not
+ * split .. 3 = a grandchild split); one iteration is the Jacobi step L_i <- max(L_i, max over the
+ * 4 edge neighbours of L_j - 1); a tile that rises to level L is refined uniformly to depth L.
+ *   tile_mask  [Ty*Tx] in/out (device): masks from noit_quadtree, updated in place
+ *   tile_level [Ty*Tx] out, optional: balanced level of every base tile
+ *   cell_level, level_hist: as in noit_quadtree, recomputed from the balanced masks (optional;
+ *              level_hist is zeroed by the call)
+ *   scales     [3] out, optional (needs level_hist): w = sum l N_l / sum N_l,
+ *              s_2 = clamp(2^(w - delta2), 0.25, 1), s_3 likewise with delta3 (Eq. 2 P:80;
+ *              the paper's delta2 = 2.2, delta3 = 3.0), fp32
+ * iterations in [0, 16] (the paper's k = 2).                                                  */
+noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32_t height, int32_t iterations,
+                                  float delta2, float delta3, uint32_t* tile_mask,
+                                  uint8_t* tile_level, uint8_t* cell_level, uint32_t* level_hist,
+                                  float* scales, void* stream);
+
 /* ---- S8 depth-based reprojection with disocclusion test (O8, A21-A23).
  * Per pixel, fp32 in a fixed order: NDC of the pixel centre and cur_depth -> M -> previous
  * pixel q and expected depth d_e; accept iff w > 0, q on screen and

@@ -21,7 +21,8 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
           4: "NOIT_ERR_NO_WEIGHTS", 5: "NOIT_ERR_CUDA", 6: "NOIT_ERR_UNSUPPORTED"}
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
-           "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_reproject"]
+           "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_balance",
+           "noit_reproject"]
 
 
 class NoitError(RuntimeError):
@@ -265,6 +266,25 @@ class Noit:
         self._check(self._L.noit_quadtree(self._ctx, _ptr(image), C.c_int32(width), C.c_int32(height),
                                           C.byref(prm), _ptr(out["tile_mask"]), _ptr(out["cell_level"]),
                                           _ptr(out["hist"]), _stream(stream)))
+        return out
+
+    # ---- NEXT-1 -----------------------------------------------------------------------
+    def quadtree_balance(self, tile_mask: torch.Tensor, width: int, height: int, iterations: int = 2,
+                         delta2: float = 2.2, delta3: float = 3.0, out=None, stream=None):
+        """In place on `tile_mask`; returns dict(tile_mask, tile_level, cell_level, hist, scales)."""
+        dev = tile_mask.device
+        Tx, Ty = (width + 63) // 64, (height + 63) // 64
+        cx, cy = (width + 7) // 8, (height + 7) // 8
+        if out is None:
+            out = dict(tile_level=torch.empty(Tx * Ty, dtype=torch.uint8, device=dev),
+                       cell_level=torch.empty(cx * cy, dtype=torch.uint8, device=dev),
+                       hist=torch.empty(4, dtype=torch.int32, device=dev),
+                       scales=torch.empty(3, dtype=torch.float32, device=dev))
+        out["tile_mask"] = tile_mask
+        self._check(self._L.noit_quadtree_balance(
+            self._ctx, C.c_int32(width), C.c_int32(height), C.c_int32(iterations), C.c_float(delta2),
+            C.c_float(delta3), _ptr(tile_mask), _ptr(out["tile_level"]), _ptr(out["cell_level"]),
+            _ptr(out["hist"]), _ptr(out["scales"]), _stream(stream)))
         return out
 
     # ---- S8 ---------------------------------------------------------------------------

@@ -78,6 +78,7 @@ void noit_destroy(noit_ctx* ctx)
     cudaFree(ctx->d_coarse_g[0]);
     cudaFree(ctx->d_coarse_g[1]);
     cudaFree(ctx->d_stage);
+    cudaFree(ctx->d_tile_depth);
     delete ctx;
 }
 

@@ -50,6 +50,53 @@ __device__ bool corner_splits(const float* __restrict__ image, int W, int H, int
     return __fmul_rn(sum, 1.0f / 6.0f) > thr;
 }
 
+// One warp: leaf level of the tile's 64 cells (2 per lane) from its mask, and the tile's
+// contribution to the histogram of leaves that hold >= 1 in-image pixel (a leaf at level l is
+// the node whose first cell has level l).  Shared by noit_quadtree and noit_quadtree_balance.
+__device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y, int W, int H, int lane,
+                                                     uint8_t* __restrict__ cell_level,
+                                                     uint32_t* __restrict__ hist)
+{
+    auto level_of_cell = [&](int cx, int cy) -> int {
+        const int c = (cx >> 2) + 2 * (cy >> 2), g = ((cx >> 1) & 1) + 2 * ((cy >> 1) & 1);
+        if (!(mask & 1u)) return 0;
+        if (!((mask >> (1 + c)) & 1u)) return 1;
+        return ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
+    };
+    const int cells_w = (W + 7) >> 3, cells_h = (H + 7) >> 3;
+    uint32_t h3 = 0;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {                        // 64 cells, 2 per lane
+        const int idx = lane + 32 * k, cx = idx & 7, cy = idx >> 3;
+        const int level = level_of_cell(cx, cy);
+        const int gx = (X >> 3) + cx, gy = (Y >> 3) + cy;
+        const bool in_image = gx < cells_w && gy < cells_h;
+        if (cell_level && in_image) cell_level[(size_t)gy * cells_w + gx] = (uint8_t)level;
+        h3 += __popc(__ballot_sync(0xffffffffu, in_image && level == 3));
+    }
+    if (!hist) return;
+    bool leaf = false;
+    int lv = 0;
+    if (lane < 21) {                                     // lane t = node t (mask bit numbering)
+        int cx = 0, cy = 0;
+        if (lane >= 5) {
+            const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+            cx = 4 * (c & 1) + 2 * (g & 1); cy = 4 * (c >> 1) + 2 * (g >> 1); lv = 2;
+        } else if (lane >= 1) {
+            cx = 4 * ((lane - 1) & 1); cy = 4 * ((lane - 1) >> 1); lv = 1;
+        }
+        leaf = X + 8 * cx < W && Y + 8 * cy < H && level_of_cell(cx, cy) == lv;
+    }
+    const uint32_t Lf = __ballot_sync(0xffffffffu, leaf);
+    if (lane == 0) {
+        const uint32_t h0 = Lf & 1u, h1 = __popc(Lf & 0x1Eu), h2 = __popc(Lf & 0x1FFFE0u);
+        if (h0) atomicAdd(hist + 0, h0);
+        if (h1) atomicAdd(hist + 1, h1);
+        if (h2) atomicAdd(hist + 2, h2);
+        if (h3) atomicAdd(hist + 3, h3);
+    }
+}
+
 __global__ void __launch_bounds__(256)
 quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint32_t var_thr,
                 float corner_thr, uint32_t* __restrict__ tile_mask, uint8_t* __restrict__ cell_level,
@@ -165,47 +212,8 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
         for (int c = 0; c < 4; ++c)
             if ((F >> (1 + c)) & 1u) mask |= (1u << (1 + c)) | (F & (0xFu << (5 + 4 * c)));
     }
-    auto level_of_cell = [&](int cx, int cy) -> int {
-        const int c = (cx >> 2) + 2 * (cy >> 2), g = ((cx >> 1) & 1) + 2 * ((cy >> 1) & 1);
-        if (!(mask & 1u)) return 0;
-        if (!((mask >> (1 + c)) & 1u)) return 1;
-        return ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
-    };
-    const int cells_w = (W + 7) >> 3, cells_h = (H + 7) >> 3;
-    uint32_t h3 = 0;
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {                        // 64 cells, 2 per lane
-        const int idx = lane + 32 * k, cx = idx & 7, cy = idx >> 3;
-        const int level = level_of_cell(cx, cy);
-        const int gx = (X >> 3) + cx, gy = (Y >> 3) + cy;
-        const bool in_image = gx < cells_w && gy < cells_h;
-        if (cell_level && in_image) cell_level[(size_t)gy * cells_w + gx] = (uint8_t)level;
-        h3 += __popc(__ballot_sync(0xffffffffu, in_image && level == 3));
-    }
     if (tile_mask && lane == 0) tile_mask[tile] = mask;
-    if (hist) {
-        // leaves with >= 1 in-image pixel: the node at level l whose first cell has level l
-        bool leaf = false;
-        int lv = 0;
-        if (lane < 21) {
-            int cx = 0, cy = 0;
-            if (lane >= 5) {
-                const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
-                cx = 4 * (c & 1) + 2 * (g & 1); cy = 4 * (c >> 1) + 2 * (g >> 1); lv = 2;
-            } else if (lane >= 1) {
-                cx = 4 * ((lane - 1) & 1); cy = 4 * ((lane - 1) >> 1); lv = 1;
-            }
-            leaf = X + 8 * cx < W && Y + 8 * cy < H && level_of_cell(cx, cy) == lv;
-        }
-        const uint32_t Lf = __ballot_sync(0xffffffffu, leaf);
-        if (lane == 0) {
-            const uint32_t h0 = Lf & 1u, h1 = __popc(Lf & 0x1Eu), h2 = __popc(Lf & 0x1FFFE0u);
-            if (h0) atomicAdd(hist + 0, h0);
-            if (h1) atomicAdd(hist + 1, h1);
-            if (h2) atomicAdd(hist + 2, h2);
-            if (h3) atomicAdd(hist + 3, h3);
-        }
-    }
+    emit_levels_and_hist(mask, X, Y, W, H, lane, cell_level, hist);
 }
 
 extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t width, int32_t height,
@@ -229,6 +237,120 @@ extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t 
                                              params->var_threshold_q, params->corner_threshold,
                                              tile_mask, cell_level, level_hist);
     ctx->launches += 1;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    return NOIT_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// NEXT-1: quadtree consistency + demand index (O10, reading A25)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int mask_depth(uint32_t mask)
+{
+    if (!(mask & 1u)) return 0;
+    if (!(mask & 0x1Eu)) return 1;
+    return (mask & 0x1FFFE0u) ? 3 : 2;
+}
+
+__global__ void __launch_bounds__(256)
+tile_depth_kernel(const uint32_t* __restrict__ tile_mask, int n, uint8_t* __restrict__ depth)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) depth[i] = (uint8_t)mask_depth(tile_mask[i]);
+}
+
+// One warp per base tile.  k Jacobi steps of L <- max(L, max over edge neighbours of L - 1)
+// equal the max-plus convolution of the initial depths with the Manhattan diamond of radius k
+// (induction on k), so each tile is finished in one pass over its diamond -- no ping-pong
+// buffers, no grid synchronisation.  A tile that rises to depth L is refined uniformly to L.
+// The last block to finish turns the histogram into w = sum l N_l / sum N_l and
+// s_p = clamp(2^(w - delta_p), 0.25, 1) (Eq. 2).
+__global__ void __launch_bounds__(128)
+balance_kernel(const uint8_t* __restrict__ depth0, int W, int H, int Tx, int Ty, int k, float delta2,
+               float delta3, uint32_t* __restrict__ tile_mask, uint8_t* __restrict__ tile_level,
+               uint8_t* __restrict__ cell_level, uint32_t* __restrict__ hist, float* __restrict__ scales,
+               uint32_t* __restrict__ ticket)
+{
+    const int lane = threadIdx.x & 31;
+    const int tile = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (tile < Tx * Ty) {
+        const int tx = tile % Tx, ty = tile / Tx;
+        // the diamond has 2k(k+1)+1 tiles; lanes stride over its rows
+        int best = 0;
+        for (int dy = -k + lane; dy <= k; dy += 32) {
+            const int y = ty + dy, r = k - abs(dy);
+            if (y < 0 || y >= Ty) continue;
+            for (int dx = -r; dx <= r; ++dx) {
+                const int x = tx + dx;
+                if (x < 0 || x >= Tx) continue;
+                best = max(best, (int)depth0[y * Tx + x] - (abs(dx) + abs(dy)));
+            }
+        }
+        best = __reduce_max_sync(0xffffffffu, best);
+        uint32_t mask = tile_mask[tile];
+        if (best >= 1) mask |= 1u;                       // every node above depth `best` splits
+        if (best >= 2) mask |= 0x1Eu;
+        if (best >= 3) mask |= 0x1FFFE0u;
+        __syncwarp();
+        if (lane == 0) {
+            tile_mask[tile] = mask;
+            if (tile_level) tile_level[tile] = (uint8_t)best;
+        }
+        emit_levels_and_hist(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist);
+    }
+    if (!scales) return;
+    // last block: demand index and Eq. 2
+    __shared__ bool last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        uint32_t n[4];
+        for (int l = 0; l < 4; ++l) n[l] = atomicAdd(hist + l, 0u);
+        const float den = (float)(n[0] + n[1] + n[2] + n[3]);
+        const float w = den > 0.f ? __fdiv_rn((float)(n[1] + 2u * n[2] + 3u * n[3]), den) : 0.f;
+        scales[0] = w;
+        scales[1] = fminf(fmaxf(exp2f(w - delta2), 0.25f), 1.0f);
+        scales[2] = fminf(fmaxf(exp2f(w - delta3), 0.25f), 1.0f);
+        *ticket = 0u;                                    // re-arm for the next call
+    }
+}
+
+extern "C" noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32_t height,
+                                             int32_t iterations, float delta2, float delta3,
+                                             uint32_t* tile_mask, uint8_t* tile_level,
+                                             uint8_t* cell_level, uint32_t* level_hist, float* scales,
+                                             void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree_balance: ctx is NULL");
+    if (!tile_mask) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance: tile_mask is NULL");
+    if (scales && !level_hist)
+        return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance: scales needs level_hist");
+    if (width <= 0 || height <= 0 || (uint64_t)width * (uint64_t)height + 1 > 0xFFFFFFFFull)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_balance: bad width/height");
+    if (iterations < 0 || iterations > 16)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_balance: iterations must be in [0, 16]");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int Tx = (width + 63) / 64, Ty = (height + 63) / 64, n = Tx * Ty;
+    if (ctx->tile_depth_cap < (size_t)n) {
+        if (ctx->d_tile_depth) {
+            NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+            NOIT_CUDA(ctx, cudaFree(ctx->d_tile_depth));
+            ctx->d_tile_depth = nullptr;
+            ctx->tile_depth_cap = 0;
+        }
+        NOIT_CUDA(ctx, cudaMalloc(&ctx->d_tile_depth, (size_t)n));
+        ctx->tile_depth_cap = (size_t)n;
+    }
+    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
+    tile_depth_kernel<<<(n + 255) / 256, 256, 0, st>>>(tile_mask, n, ctx->d_tile_depth);
+    balance_kernel<<<(n + 3) / 4, 128, 0, st>>>(ctx->d_tile_depth, width, height, Tx, Ty, iterations,
+                                                delta2, delta3, tile_mask, tile_level, cell_level,
+                                                level_hist, scales, ctx->d_counters + 2);
+    ctx->launches += 2;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
 }

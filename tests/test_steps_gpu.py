@@ -218,6 +218,53 @@ def test_fallback_resolve_on_reject_list(noit):
 # -------------------------------------------------------------------------------------------
 # ABI error behaviour: host-checkable errors come back before any launch
 # -------------------------------------------------------------------------------------------
+# -------------------------------------------------------------------------------------------
+# NEXT-1: quadtree consistency + demand index (O10)
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,W,H,k", [(0, 1920, 1080, 2), (1, 3840, 2160, 2), (2, 40, 40, 2),
+                                        (3, 300, 50, 2), (4, 1000, 700, 1), (5, 1000, 700, 5),
+                                        (6, 640, 640, 0)])
+def test_quadtree_balance_random_masks(noit, seed, W, H, k):
+    from test_oracle_pins import _random_valid_masks
+    rng = np.random.default_rng(seed)
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    m = _random_valid_masks(rng, Tx * Ty)
+    ref = oracle.quadtree_balance(m, W, H, iterations=k)
+    ctx = noit.Noit()
+    d_mask = torch.from_numpy(m.view(np.int32).copy()).cuda()
+    got = ctx.quadtree_balance(d_mask, W, H, iterations=k)
+    got2 = None
+    if k == 2:                                         # balanced input: a second call is a no-op
+        got2 = ctx.quadtree_balance(d_mask.clone(), W, H, iterations=k)
+    assert np.array_equal(u32(got["tile_mask"]), ref["tile_mask"])
+    assert np.array_equal(got["tile_level"].cpu().numpy(), ref["tile_level"])
+    assert np.array_equal(got["cell_level"].cpu().numpy(), ref["cell_level"])
+    assert np.array_equal(u32(got["hist"]), ref["hist"])
+    assert np.max(np.abs(got["scales"].cpu().numpy().astype(np.float64) - ref["scales"])) <= 1e-6
+    if got2 is not None:
+        assert np.array_equal(u32(got2["tile_mask"]), ref["tile_mask"])
+        assert np.array_equal(u32(got2["hist"]), ref["hist"])
+
+
+def test_quadtree_then_balance_on_cfg4(noit, cfg4_small):
+    """S6 -> NEXT-1 chained on a resolved frame: masks from noit_quadtree, balanced in place."""
+    sc = cfg4_small
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    fb = noit.DeviceFragBuf.from_host(sc.full)
+    img = ctx.resolve(fb, BG)["final"]
+    qt = ctx.quadtree(img, fb.width, fb.height, var_threshold_q=6)
+    ref_qt = oracle.quadtree(img.cpu().numpy(), fb.width, fb.height, 0, 6)
+    ref = oracle.quadtree_balance(ref_qt["tile_mask"], fb.width, fb.height)
+    got = ctx.quadtree_balance(qt["tile_mask"], fb.width, fb.height)
+    for k in ("tile_mask", "hist"):
+        assert np.array_equal(u32(got[k]), ref[k]), k
+    for k in ("tile_level", "cell_level"):
+        assert np.array_equal(got[k].cpu().numpy(), ref[k]), k
+    lv = ref["tile_level"].reshape((fb.height + 63) // 64, (fb.width + 63) // 64).astype(int)
+    assert np.all(np.abs(np.diff(lv, axis=0)) <= 1) and np.all(np.abs(np.diff(lv, axis=1)) <= 1)
+    assert np.max(np.abs(got["scales"].cpu().numpy() - ref["scales"])) <= 1e-6
+
+
 def test_abi_errors(noit, cfg1_scene):
     import ctypes as C
     sc = cfg1_scene
