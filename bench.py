@@ -6,6 +6,7 @@ complexity workload (BASELINE.json configs[2], "cfg3", plus the half/quarter buf
 primitives):
    1. noit_resolve   plain fused resolve of the frame (S1-S5)          <- dominant kernel
    2. noit_quadtree  colour-variance tiles of its result (S6)
+      + noit_quadtree_balance  2:1 tile consistency, histogram, demand index, Eq. 2 (NEXT-1)
    3. noit_resolve   adaptive resolve guided by those tiles (S7)
    4. noit_reproject previous result under a small camera motion (S8)
    5. noit_resolve   fallback resolve of the rejected pixels (S9)
@@ -154,6 +155,7 @@ def oracle_step(oracle, sc, w_eff, M, state):
     W, H = fbh.width, fbh.height
     r = oracle.resolve(fbh, w_eff, BG)
     qt = oracle.quadtree(r["final"], W, H, 0, 6)
+    qt = oracle.quadtree_balance(qt["tile_mask"], W, H)
     oracle.resolve(fbh, w_eff, BG, half=sc.half, quarter=sc.quarter, cell_level=qt["cell_level"])
     rp = oracle.reproject(W, H, M, 1e-3, BG, r["trans"], r["depth1"], r["depth1"])
     out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
@@ -224,19 +226,21 @@ def run_ours(args):
     plain = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
     adapt = dict(final=torch.empty((P, 4), **f32))
     qt = None
+    bal = None
     rp = None
     d_plain = ctx.make_resolve_desc(fb, BG, plain["trans"], plain["final"], plain["depth1"])
     stream = torch.cuda.current_stream()
-    names = ["resolve", "quadtree", "adaptive", "reproject", "fallback"]
+    names = ["resolve", "quadtree+balance", "adaptive", "reproject", "fallback"]
 
     def step(ev=None):
-        nonlocal qt, rp
+        nonlocal qt, bal, rp
         if ev: ev[0].record(stream)
         ctx.resolve_desc(d_plain)
         if ev: ev[1].record(stream)
         qt = ctx.quadtree(plain["final"], W, H, noit.QT_VARIANCE, 6, out=qt)
+        bal = ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal)
         if ev: ev[2].record(stream)
-        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=qt["cell_level"])
+        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=bal["cell_level"])
         if ev: ev[3].record(stream)
         rp = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"], out=rp)
         if ev: ev[4].record(stream)
@@ -292,7 +296,8 @@ def run_ours(args):
     e2e_ms = max_over_ranks(dist, e0.elapsed_time(e1) / e2e_steps, dev)
     clocks = sampler.stop() if rank == 0 else None
     rejected = int(rp["reject_count"].item())
-    hist = qt["hist"].cpu().numpy().view(np.uint32).tolist()
+    hist = bal["hist"].cpu().numpy().view(np.uint32).tolist()
+    scales = [float(v) for v in bal["scales"].cpu().numpy()]
 
     if rank == 0:
         peak, peak_src = peaks()
@@ -318,7 +323,7 @@ def run_ours(args):
                     "h2d_bytes_per_step": 4 * (P + 1) + 12 * F, "d2h_bytes_per_step": 16 * P,
                     "ms_per_step": e2e_ms},
             "gpu_launches": launches, "clocks": clocks,
-            "tile_hist": hist, "rejected_fraction": rejected / P,
+            "tile_hist": hist, "demand_index_and_scales": scales, "rejected_fraction": rejected / P,
         }
         if world == 1 and not args.no_cpu_baseline:
             rec["cpu_baseline"] = cpu_baseline(sc)
