@@ -219,6 +219,99 @@ def test_fallback_resolve_on_reject_list(noit):
 # ABI error behaviour: host-checkable errors come back before any launch
 # -------------------------------------------------------------------------------------------
 # -------------------------------------------------------------------------------------------
+# BASELINE.json configs[3] and configs[4] at FULL size, in the call sequence bench.py times
+# -------------------------------------------------------------------------------------------
+def test_cfg4_full_size_adaptive_frame(noit):
+    """1920x1080 adaptive tiling (cfg4): resolve -> quadtree -> balance -> adaptive resolve."""
+    sc = noit_scenes.cfg4(0)
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    W, H = fb.width, fb.height
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    plain = ctx.resolve(fb, BG)
+    check_resolve(noit, sc.full, sc.weights, sc.mlp_precision, plain)
+    img = plain["final"].cpu().numpy()
+    qt = ctx.quadtree(plain["final"], W, H, 0, 6)
+    ref_qt = oracle.quadtree(img, W, H, 0, 6)                                  # same image (A16)
+    qt_equal(qt, ref_qt)
+    coarse = np.isin(ref_qt["cell_level"], (0, 1)).mean()
+    assert 0.3 < coarse < 0.6, coarse                                          # ~50 % smooth regions
+    bal = ctx.quadtree_balance(qt["tile_mask"], W, H)
+    ref_bal = oracle.quadtree_balance(ref_qt["tile_mask"], W, H)
+    assert np.array_equal(u32(bal["tile_mask"]), ref_bal["tile_mask"])
+    assert np.array_equal(bal["cell_level"].cpu().numpy(), ref_bal["cell_level"])
+    assert np.array_equal(u32(bal["hist"]), ref_bal["hist"])
+    got = ctx.resolve(fb, BG, half=hb, quarter=qb, cell_level=bal["cell_level"])
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    ref = oracle.resolve(sc.full, w_eff, BG, half=sc.half, quarter=sc.quarter,
+                         cell_level=ref_bal["cell_level"])
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    lay = oracle.build_features(sc.full)
+    mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=extra)
+        assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
+
+
+def run_sequence(noit, seq, n_frames):
+    """cfg5's schedule: even frames are resolved, odd frames reuse the previous transparency
+    result by reprojection (mode A: cur_depth = prev_depth) and resolve the rejected pixels."""
+    W, H = seq.width, seq.height
+    ctx = noit.Noit(seq.weights, seq.mlp_precision)
+    w_eff = oracle.effective_weights(seq.weights, seq.mlp_precision)
+    prev = None
+    fractions = []
+    for t in range(n_frames):
+        fbh = seq.frame(t)
+        fb = noit.DeviceFragBuf.from_host(fbh)
+        if t % 2 == 0:
+            got = ctx.resolve(fb, seq.background)
+            check_resolve(noit, fbh, seq.weights, seq.mlp_precision, got,
+                          ref=oracle.resolve(fbh, w_eff, seq.background))
+            prev = got
+            continue
+        M = seq.reproject_matrix(t)
+        p_t, p_d = prev["trans"].cpu().numpy(), prev["depth1"].cpu().numpy()
+        rp = ctx.reproject(W, H, M, seq.depth_threshold, seq.background, prev["trans"], prev["depth1"],
+                           prev["depth1"])
+        ref_rp = oracle.reproject(W, H, M, seq.depth_threshold, seq.background, p_t, p_d, p_d)
+        acc = rp["accept"].cpu().numpy()
+        assert np.array_equal(acc, ref_rp["accept"])                           # bit-exact mask
+        n = int(rp["reject_count"].item())
+        assert n == ref_rp["reject_count"] == int((acc == 0).sum())
+        assert np.array_equal(np.sort(u32(rp["reject_list"])[:n]), np.sort(ref_rp["reject_list"]))
+        out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+        ctx.resolve(fb, seq.background, out=out, pixel_list=rp["reject_list"],
+                    pixel_count=rp["reject_count"])
+        ref = dict(trans=ref_rp["trans"], final=ref_rp["final"], depth1=ref_rp["depth"])
+        oracle.resolve(fbh, w_eff, seq.background, pixel_list=ref_rp["reject_list"], out=ref)
+        m = acc.astype(bool)
+        assert np.array_equal(out["trans"].cpu().numpy()[m], ref["trans"][m])  # accepted: bit copies
+        assert np.array_equal(out["depth1"].cpu().numpy(), ref["depth1"])
+        lay = oracle.build_features(fbh)
+        mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+        extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+        for k in ("trans", "final"):
+            close(out[k].cpu().numpy(), ref[k], extra=extra)
+        fractions.append(n / (W * H))
+    return fractions
+
+
+def test_cfg5_sequence_reduced_all_eight_frames(noit):
+    """The whole 8-frame schedule of cfg5 on a 960x540 version of the same scene and camera path."""
+    seq = noit_scenes.cfg5(0, W=960, H=540)
+    fr = run_sequence(noit, seq, 8)
+    assert len(fr) == 4 and all(0.0 < f < 0.5 for f in fr), fr
+
+
+def test_cfg5_full_size_first_two_frames(noit):
+    """3840x2160: frame 0 resolved, frame 1 reprojected + fallback (BASELINE.json configs[4])."""
+    seq = noit_scenes.cfg5(0)
+    fr = run_sequence(noit, seq, 2)
+    assert 0.0 < fr[0] < 0.5, fr
+
+
+# -------------------------------------------------------------------------------------------
 # NEXT-1: quadtree consistency + demand index (O10)
 # -------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("seed,W,H,k", [(0, 1920, 1080, 2), (1, 3840, 2160, 2), (2, 40, 40, 2),
