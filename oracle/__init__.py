@@ -161,6 +161,26 @@ def quadtree_balance(tile_mask: np.ndarray, width: int, height: int, iterations:
     return out
 
 
+def quadtree_temporal(image: np.ndarray, width: int, height: int, prev_mask=None, metric: int = 0,
+                      var_split: int = 6, var_merge: int = 3, corner_split: float = 0.02,
+                      corner_merge: float = 0.01, max_step: int = 1) -> dict:
+    """O11: quadtree with split / merge hysteresis against the previous frame's masks and at most
+    `max_step` levels of change per base tile and frame."""
+    img = _chk(np.ascontiguousarray(image, np.float32), np.float32, width * height * 4)
+    Tx, Ty = (width + 63) // 64, (height + 63) // 64
+    cx, cy = (width + 7) // 8, (height + 7) // 8
+    prev = None if prev_mask is None else _chk(np.ascontiguousarray(prev_mask, np.uint32), np.uint32, Tx * Ty)
+    out = dict(tile_mask=np.zeros(Tx * Ty, np.uint32), cell_level=np.zeros(cx * cy, np.uint8),
+               hist=np.zeros(4, np.uint32))
+    rc = lib().oracle_quadtree_temporal(_p(img), C.c_int32(width), C.c_int32(height), C.c_int32(metric),
+                                        C.c_uint32(var_split), C.c_uint32(var_merge),
+                                        C.c_float(corner_split), C.c_float(corner_merge),
+                                        C.c_int32(max_step), None if prev is None else _p(prev),
+                                        _p(out["tile_mask"]), _p(out["cell_level"]), _p(out["hist"]))
+    assert rc == 0
+    return out
+
+
 def reproject(width, height, M, depth_threshold, background, prev_trans, prev_depth, cur_depth,
               out_trans=None, out_depth=None, out_final=None) -> dict:
     P = width * height

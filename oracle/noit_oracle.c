@@ -538,6 +538,37 @@ static int mask_depth(uint32_t mask)
     return 3;
 }
 
+/* leaf level of every 8x8 cell and the histogram of leaves that hold >= 1 in-image pixel,      */
+/* recounted from the 21-bit masks alone                                                       */
+static void levels_and_hist_from_masks(int32_t width, int32_t height, const uint32_t *tile_mask,
+                                       uint8_t *cell_level, uint64_t h[4])
+{
+    int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
+    int cells_x = (width + 7) / 8, cells_y = (height + 7) / 8;
+    h[0] = h[1] = h[2] = h[3] = 0;
+    for (int ty = 0; ty < Ty; ++ty)
+        for (int tx = 0; tx < Tx; ++tx) {
+            uint32_t mask = tile_mask[ty * Tx + tx];
+            int X = tx * 64, Y = ty * 64;
+            for (int v = 0; v < 8; ++v)
+                for (int u = 0; u < 8; ++u) {
+                    int c = (u >> 2) + 2 * (v >> 2), g = ((u >> 1) & 1) + 2 * ((v >> 1) & 1);
+                    int level = 0;
+                    if (mask & 1u) {
+                        level = 1;
+                        if ((mask >> (1 + c)) & 1u) level = ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
+                    }
+                    int cxg = X / 8 + u, cyg = Y / 8 + v;
+                    if (cxg >= cells_x || cyg >= cells_y) continue;
+                    if (cell_level) cell_level[cyg * cells_x + cxg] = (uint8_t)level;
+                    /* a leaf is counted at its first (top-left) cell, which is in the image  */
+                    /* whenever the leaf holds an in-image pixel                              */
+                    int span = 8 >> level;              /* leaf side in cells */
+                    if (u % span == 0 && v % span == 0) h[level] += 1;
+                }
+        }
+}
+
 int32_t oracle_quadtree_balance(int32_t width, int32_t height, int32_t iterations, float delta2,
                                 float delta3, uint32_t *tile_mask, uint8_t *tile_level,
                                 uint8_t *cell_level, uint32_t *hist, float *scales)
@@ -560,33 +591,17 @@ int32_t oracle_quadtree_balance(int32_t width, int32_t height, int32_t iteration
             }
         int *t = cur; cur = nxt; nxt = t;
     }
-    uint64_t h[4] = {0, 0, 0, 0};
-    for (int ty = 0; ty < Ty; ++ty)
-        for (int tx = 0; tx < Tx; ++tx) {
-            int i = ty * Tx + tx, L = cur[i], X = tx * 64, Y = ty * 64;
-            uint32_t mask = tile_mask[i];
-            if (L >= 1) mask |= 1u;                      /* every node above depth L splits */
-            if (L >= 2) mask |= 0x1Eu;
-            if (L >= 3) mask |= 0x1FFFE0u;
-            tile_mask[i] = mask;
-            if (tile_level) tile_level[i] = (uint8_t)L;
-            for (int v = 0; v < 8; ++v)
-                for (int u = 0; u < 8; ++u) {
-                    int c = (u >> 2) + 2 * (v >> 2), g = ((u >> 1) & 1) + 2 * ((v >> 1) & 1);
-                    int level = 0;
-                    if (mask & 1u) {
-                        level = 1;
-                        if ((mask >> (1 + c)) & 1u) level = ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
-                    }
-                    int cxg = X / 8 + u, cyg = Y / 8 + v;
-                    if (cxg >= cells_x || cyg >= cells_y) continue;
-                    if (cell_level) cell_level[cyg * cells_x + cxg] = (uint8_t)level;
-                    /* a leaf is counted at its first (top-left) cell, which is in the image  */
-                    /* whenever the leaf holds an in-image pixel                              */
-                    int span = 8 >> level;              /* leaf side in cells */
-                    if (u % span == 0 && v % span == 0) h[level] += 1;
-                }
-        }
+    for (int i = 0; i < n; ++i) {
+        int L = cur[i];
+        uint32_t mask = tile_mask[i];
+        if (L >= 1) mask |= 1u;                          /* every node above depth L splits */
+        if (L >= 2) mask |= 0x1Eu;
+        if (L >= 3) mask |= 0x1FFFE0u;
+        tile_mask[i] = mask;
+        if (tile_level) tile_level[i] = (uint8_t)L;
+    }
+    uint64_t h[4];
+    levels_and_hist_from_masks(width, height, tile_mask, cell_level, h);
     if (hist) for (int k = 0; k < 4; ++k) hist[k] = (uint32_t)h[k];
     if (scales) {
         double num = 0.0, den = 0.0;
@@ -598,6 +613,114 @@ int32_t oracle_quadtree_balance(int32_t width, int32_t height, int32_t iteration
         scales[0] = (float)w; scales[1] = (float)s2; scales[2] = (float)s3;
     }
     free(cur); free(nxt);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
+/* O11 temporal tile state ("tiles computed in frame F_t guide ...     */
+/* F_t+1", P:61 split / merge thresholds, "tiles may change by only one level per frame"). */
+/* Reading A26: a node that was NOT split in the previous frame splits iff          */
+/* metric > split threshold; a node that WAS split merges iff metric < merge threshold, with    */
+/* merge <= split (a hysteresis band in which a node keeps its state; P:61's sentence "split    */
+/* thresholds being smaller than the merge thresholds" read literally would make a node in the  */
+/* band flip every frame, against its stated purpose).  Evaluation is top-down as in O6.  Then  */
+/* the depth of each base tile is limited to prev_depth +- max_step: a deeper tree is truncated */
+/* (bits below the limit cleared), a shallower one is refined uniformly to the limit.           */
+/* metric vs threshold: above = 1 -> metric > thr, above = 0 -> metric < thr                    */
+static int node_cmp(const qt_args *a, int x0, int y0, int side, uint32_t var_thr, float corner_thr,
+                    int above)
+{
+    int x1 = x0 + side, y1 = y0 + side;
+    if (x1 > a->width) x1 = a->width;
+    if (y1 > a->height) y1 = a->height;
+    if (a->metric == 0) {
+        uint64_t n = 0, s1[3] = {0, 0, 0}, s2[3] = {0, 0, 0};
+        for (int y = y0; y < y1; ++y)
+            for (int x = x0; x < x1; ++x) {
+                const float *px = a->image + 4 * ((size_t)y * a->width + x);
+                for (int c = 0; c < 3; ++c) {
+                    uint64_t q = quant8(px[c]);
+                    s1[c] += q;
+                    s2[c] += q * q;
+                }
+                ++n;
+            }
+        uint64_t lhs = 0, rhs = (uint64_t)var_thr * n * n;
+        for (int c = 0; c < 3; ++c) lhs += n * s2[c] - s1[c] * s1[c];
+        return above ? lhs > rhs : lhs < rhs;
+    }
+    int xs[4] = {x0, x1 - 1, x0, x1 - 1}, ys[4] = {y0, y0, y1 - 1, y1 - 1};
+    static const int pa[6] = {0, 0, 0, 1, 1, 2}, pb[6] = {1, 2, 3, 2, 3, 3};
+    float sum = 0.0f;
+    for (int k = 0; k < 6; ++k) {
+        const float *A = a->image + 4 * ((size_t)ys[pa[k]] * a->width + xs[pa[k]]);
+        const float *B = a->image + 4 * ((size_t)ys[pb[k]] * a->width + xs[pb[k]]);
+        float dr = A[0] - B[0], dg = A[1] - B[1], db = A[2] - B[2];
+        float sq = dr * dr;
+        sq = sq + dg * dg;
+        sq = sq + db * db;
+        float root = sqrtf(sq);
+        sum = k == 0 ? root : sum + root;
+    }
+    float D = sum * (1.0f / 6.0f);
+    return above ? D > corner_thr : D < corner_thr;
+}
+
+typedef struct {
+    uint32_t var_split, var_merge;
+    float corner_split, corner_merge;
+} hyst_args;
+
+/* split state of a node this frame given its state in the previous frame                       */
+static int node_state(const qt_args *a, const hyst_args *h, int x0, int y0, int side, int was_split)
+{
+    if (x0 >= a->width || y0 >= a->height) return 0;     /* wholly outside the image (A17) */
+    if (was_split) return !node_cmp(a, x0, y0, side, h->var_merge, h->corner_merge, 0);
+    return node_cmp(a, x0, y0, side, h->var_split, h->corner_split, 1);
+}
+
+int32_t oracle_quadtree_temporal(const float *image, int32_t width, int32_t height, int32_t metric,
+                                 uint32_t var_split, uint32_t var_merge, float corner_split,
+                                 float corner_merge, int32_t max_step, const uint32_t *prev_mask,
+                                 uint32_t *tile_mask, uint8_t *cell_level, uint32_t *hist)
+{
+    qt_args a = {image, width, height, metric, var_split, corner_split};
+    hyst_args hy = {var_split, var_merge, corner_split, corner_merge};
+    int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
+    for (int ty = 0; ty < Ty; ++ty)
+        for (int tx = 0; tx < Tx; ++tx) {
+            int X = tx * 64, Y = ty * 64;
+            uint32_t prev = prev_mask ? prev_mask[ty * Tx + tx] : 0u, mask = 0;
+            if (node_state(&a, &hy, X, Y, 64, (int)(prev & 1u))) {
+                mask |= 1u;
+                for (int c = 0; c < 4; ++c) {
+                    int cx = X + 32 * (c & 1), cy = Y + 32 * (c >> 1);
+                    if (!node_state(&a, &hy, cx, cy, 32, (int)((prev >> (1 + c)) & 1u))) continue;
+                    mask |= 1u << (1 + c);
+                    for (int g = 0; g < 4; ++g) {
+                        int gx = cx + 16 * (g & 1), gy = cy + 16 * (g >> 1);
+                        if (node_state(&a, &hy, gx, gy, 16, (int)((prev >> (5 + 4 * c + g)) & 1u)))
+                            mask |= 1u << (5 + 4 * c + g);
+                    }
+                }
+            }
+            if (prev_mask && max_step > 0) {             /* at most max_step levels per frame */
+                int pd = mask_depth(prev), d = mask_depth(mask);
+                if (d > pd + max_step) {
+                    int lim = pd + max_step;             /* truncate below depth lim */
+                    mask &= lim == 0 ? 0u : (lim == 1 ? 0x1u : (lim == 2 ? 0x1Fu : 0x1FFFFFu));
+                } else if (d < pd - max_step) {
+                    int lim = pd - max_step;             /* refine uniformly to depth lim */
+                    mask |= lim >= 1 ? 1u : 0u;
+                    mask |= lim >= 2 ? 0x1Eu : 0u;
+                    mask |= lim >= 3 ? 0x1FFFE0u : 0u;
+                }
+            }
+            tile_mask[ty * Tx + tx] = mask;
+        }
+    uint64_t h[4];
+    levels_and_hist_from_masks(width, height, tile_mask, cell_level, h);
+    if (hist) for (int k = 0; k < 4; ++k) hist[k] = (uint32_t)h[k];
     return 0;
 }
 

@@ -734,3 +734,85 @@ def test_demand_index_and_eq2_fixed_points():
     r = oracle.quadtree_balance(np.full(6, FULL[2], np.uint32), 3 * 64, 2 * 64)       # w = 2
     assert r["scales"][0] == 2.0 and r["scales"][2] == 0.5
     assert abs(r["scales"][1] - 0.8705505632961241) < 1e-6                            # 2^-0.2
+
+
+# -------------------------------------------------------------------------------------------
+# O11: temporal tile state (split / merge hysteresis, at most one level of change per frame;
+# PAPER.md:55, :61, :63; reading A26)
+# -------------------------------------------------------------------------------------------
+def _one_white_pixel(W, H, x, y):
+    img = np.zeros((H * W, 4), np.float32)
+    img[y * W + x, :3] = 1.0
+    return img
+
+
+@pytest.mark.parametrize("metric", [0, 1])
+def test_temporal_without_history_is_the_plain_quadtree(metric):
+    rng = np.random.default_rng(40 + metric)
+    W, H = 200, 136
+    img = rng.random((H * W, 4)).astype(np.float32) * np.float32(0.3)
+    img[: W * 40] = 0.5                                                       # a flat band too
+    a = oracle.quadtree(img, W, H, metric, 600, 0.12)
+    b = oracle.quadtree_temporal(img, W, H, None, metric, 600, 200, 0.12, 0.05, max_step=1)
+    for k in ("tile_mask", "cell_level", "hist"):
+        assert np.array_equal(a[k], b[k]), k
+    # equal thresholds and no step limit: the history cannot matter (no metric sits on the threshold)
+    prev = _random_valid_masks(rng, a["tile_mask"].size)
+    c = oracle.quadtree_temporal(img, W, H, prev, 1, 600, 600, 0.12, 0.12, max_step=0)
+    assert np.array_equal(c["tile_mask"], oracle.quadtree(img, W, H, 1, 600, 0.12)["tile_mask"])
+
+
+def test_temporal_constant_image_merges_one_level_per_frame():
+    W, H = 192, 128
+    img = np.full((H * W, 4), 0.5, np.float32)
+    m = np.full(6, FULL[3], np.uint32)
+    seen = []
+    for _ in range(4):
+        r = oracle.quadtree_temporal(img, W, H, m)
+        m = r["tile_mask"]
+        seen.append((int(m[0]), r["hist"].tolist()))
+    assert seen == [(FULL[2], [0, 0, 96, 0]), (FULL[1], [0, 24, 0, 0]), (0, [6, 0, 0, 0]), (0, [6, 0, 0, 0])]
+    r = oracle.quadtree_temporal(img, W, H, np.full(6, FULL[3], np.uint32), max_step=0)
+    assert not r["tile_mask"].any()                                           # no limit: all the way
+
+
+def test_temporal_hysteresis_band_keeps_the_previous_state():
+    """One white pixel in a black 64x64 tile: summed variance of a node with n pixels is
+    3 (n-1)/n^2 255^2 -> root 47.6, its 32x32 child 190.3, the 16x16 grandchild 759.0."""
+    W = H = 64
+    img = _one_white_pixel(W, H, 5, 5)
+    for n, v in ((4096, 47.6), (1024, 190.3), (256, 759.0)):
+        assert abs(3 * (n - 1) / n ** 2 * 255 ** 2 - v) < 0.05
+    q = lambda prev, **kw: int(oracle.quadtree_temporal(
+        img, W, H, None if prev is None else np.array([prev], np.uint32), 0, 60, 30, **kw)["tile_mask"][0])
+    assert q(None) == 0                      # 47.6 is not above the split threshold 60
+    assert q(0) == 0                         # unsplit root inside the band [30, 60]: stays unsplit
+    assert q(0x1, max_step=0) == 0x23        # split root inside the band: stays split; the path
+    #                                          to the pixel (190 > 60, 759 > 60) splits below it
+    assert q(0x1) == 0x3                     # ... but only one level deeper per frame (1 -> 2)
+    assert q(0x3) == 0x23                    # next frame: depth 3
+    assert q(0x1F, max_step=0) == 0x23       # children without the pixel (variance 0 < 30) merge
+    q2 = lambda prev: int(oracle.quadtree_temporal(
+        img, W, H, np.array([prev], np.uint32), 0, 40, 30, max_step=0)["tile_mask"][0])
+    assert q2(0) == 0x23                     # 47.6 > 40: splits whatever the history
+    q3 = lambda prev: int(oracle.quadtree_temporal(
+        img, W, H, np.array([prev], np.uint32), 0, 60, 50, max_step=0)["tile_mask"][0])
+    assert q3(0x23) == 0                     # 47.6 < 50: the root merges and takes its subtree along
+
+
+def test_temporal_step_limit_and_mask_validity_random():
+    rng = np.random.default_rng(44)
+    W, H = 520, 330
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    img = (rng.random((H * W, 4)) * rng.random((H * W, 1)) ** 3).astype(np.float32)
+    prev = _random_valid_masks(rng, Tx * Ty)
+    r = oracle.quadtree_temporal(img, W, H, prev, 0, 2500, 1500, max_step=1)
+    for a, b in zip(prev, r["tile_mask"]):
+        a, b = int(a), int(b)
+        assert abs(_depth(a) - _depth(b)) <= 1
+        for c in range(4):
+            if b >> (1 + c) & 1:
+                assert b & 1
+            for g in range(4):
+                if b >> (5 + 4 * c + g) & 1:
+                    assert b >> (1 + c) & 1
