@@ -158,6 +158,26 @@ noit_status noit_quadtree(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t 
                           int32_t height, const noit_qt_params* params, uint32_t* tile_mask,
                           uint8_t* cell_level, uint32_t* level_hist, void* stream);
 
+/* ---- NEXT-2: temporal tile state ("tiles computed in frame F_t guide ... F_t+1", P:61
+ * split / merge thresholds, "tiles may change by only one level per frame"; O11, A26).
+ * noit_quadtree with a memory: a node that was NOT split in prev_tile_mask splits iff
+ * metric > split threshold; a node that WAS split merges iff metric < merge threshold
+ * (merge <= split: inside the band a node keeps its state).  Then the depth of every base tile
+ * is limited to its previous depth +- max_level_step (deeper: truncated; shallower: refined
+ * uniformly).  prev_tile_mask == NULL: no history, identical to noit_quadtree with the split
+ * thresholds.  prev_tile_mask must not alias tile_mask.  max_level_step in [0, 3], 0 = no
+ * limit (the paper: 1).  Outputs as in noit_quadtree.                                       */
+typedef struct {
+    int32_t metric;
+    uint32_t var_split_q, var_merge_q;      /* summed-over-channels variance, 8-bit units squared */
+    float corner_split, corner_merge;
+    int32_t max_level_step;
+} noit_qt_temporal_params;
+noit_status noit_quadtree_temporal(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t width,
+                                   int32_t height, const noit_qt_temporal_params* params,
+                                   const uint32_t* prev_tile_mask, uint32_t* tile_mask,
+                                   uint8_t* cell_level, uint32_t* level_hist, void* stream);
+
 /* ---- NEXT-1: quadtree consistency + demand index (O10, reading A25).
  * "neighboring tiles may differ by at most one refinement level ... two relaxation iterations
  * (k=2) are sufficient": the level of a base tile is the depth of its subtree (0 = not

@@ -21,7 +21,8 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
           4: "NOIT_ERR_NO_WEIGHTS", 5: "NOIT_ERR_CUDA", 6: "NOIT_ERR_UNSUPPORTED"}
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
-           "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_balance",
+           "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
+           "noit_quadtree_balance",
            "noit_reproject"]
 
 
@@ -53,6 +54,11 @@ class ResolveDescC(C.Structure):
 class QtParamsC(C.Structure):
     _fields_ = [("metric", C.c_int32), ("var_threshold_q", C.c_uint32),
                 ("corner_threshold", C.c_float)]
+
+
+class QtTemporalParamsC(C.Structure):
+    _fields_ = [("metric", C.c_int32), ("var_split_q", C.c_uint32), ("var_merge_q", C.c_uint32),
+                ("corner_split", C.c_float), ("corner_merge", C.c_float), ("max_level_step", C.c_int32)]
 
 
 class ReprojectDescC(C.Structure):
@@ -266,6 +272,25 @@ class Noit:
         self._check(self._L.noit_quadtree(self._ctx, _ptr(image), C.c_int32(width), C.c_int32(height),
                                           C.byref(prm), _ptr(out["tile_mask"]), _ptr(out["cell_level"]),
                                           _ptr(out["hist"]), _stream(stream)))
+        return out
+
+    # ---- NEXT-2 -----------------------------------------------------------------------
+    def quadtree_temporal(self, image: torch.Tensor, width: int, height: int, prev_mask=None,
+                          metric: int = QT_VARIANCE, var_split: int = 6, var_merge: int = 3,
+                          corner_split: float = 0.02, corner_merge: float = 0.01, max_step: int = 1,
+                          out=None, stream=None):
+        assert image.dtype == torch.float32 and image.is_contiguous()
+        dev = image.device
+        Tx, Ty = (width + 63) // 64, (height + 63) // 64
+        cx, cy = (width + 7) // 8, (height + 7) // 8
+        if out is None:
+            out = dict(tile_mask=torch.empty(Tx * Ty, dtype=torch.int32, device=dev),
+                       cell_level=torch.empty(cx * cy, dtype=torch.uint8, device=dev),
+                       hist=torch.empty(4, dtype=torch.int32, device=dev))
+        prm = QtTemporalParamsC(metric, var_split, var_merge, corner_split, corner_merge, max_step)
+        self._check(self._L.noit_quadtree_temporal(
+            self._ctx, _ptr(image), C.c_int32(width), C.c_int32(height), C.byref(prm), _ptr(prev_mask),
+            _ptr(out["tile_mask"]), _ptr(out["cell_level"]), _ptr(out["hist"]), _stream(stream)))
         return out
 
     # ---- NEXT-1 -----------------------------------------------------------------------

@@ -13,20 +13,40 @@ __device__ __forceinline__ uint32_t quant8(float c)
 
 struct Moments { uint32_t n, s1[3], s2[3]; };
 
-__device__ __forceinline__ bool variance_splits(const Moments& m, uint32_t thr)
+// depth of a base tile's subtree: 0 = not split .. 3 = a grandchild split
+__device__ __forceinline__ int mask_depth(uint32_t mask)
+{
+    if (!(mask & 1u)) return 0;
+    if (!(mask & 0x1Eu)) return 1;
+    return (mask & 0x1FFFE0u) ? 3 : 2;
+}
+
+
+// NEXT-2 (O11, A26): the previous frame's masks make the split test a hysteresis: a node that
+// was not split splits iff metric > split threshold, a node that was split merges iff
+// metric < merge threshold.  prev_mask == nullptr: every node "was not split" (plain O6).
+struct QtTemporal {
+    const uint32_t* prev_mask;
+    uint32_t var_merge;
+    float corner_merge;
+    int max_step;                  // levels a base tile may change per frame (0 = unlimited)
+};
+
+__device__ __forceinline__ bool variance_splits(const Moments& m, uint32_t split_thr, uint32_t merge_thr,
+                                                bool was_split)
 {
     if (m.n == 0) return false;                       // wholly outside the image (A17)
     const uint64_t n = m.n;
     uint64_t lhs = 0;
 #pragma unroll
     for (int c = 0; c < 3; ++c) lhs += n * (uint64_t)m.s2[c] - (uint64_t)m.s1[c] * (uint64_t)m.s1[c];
-    return lhs > (uint64_t)thr * n * n;
+    return was_split ? !(lhs < (uint64_t)merge_thr * n * n) : lhs > (uint64_t)split_thr * n * n;
 }
 
 // Corner metric D (A14): mean pairwise Euclidean RGB distance of the 4 corner pixels
 // of the node's in-image rectangle; fp32, pairs (01,02,03,12,13,23), nothing contracted.
 __device__ bool corner_splits(const float* __restrict__ image, int W, int H, int x0, int y0, int side,
-                              float thr)
+                              float split_thr, float merge_thr, bool was_split)
 {
     const int x1 = min(x0 + side, W), y1 = min(y0 + side, H);
     if (x0 >= x1 || y0 >= y1) return false;
@@ -47,7 +67,8 @@ __device__ bool corner_splits(const float* __restrict__ image, int W, int H, int
         const float root = __fsqrt_rn(s);
         sum = k == 0 ? root : __fadd_rn(sum, root);
     }
-    return __fmul_rn(sum, 1.0f / 6.0f) > thr;
+    const float D = __fmul_rn(sum, 1.0f / 6.0f);
+    return was_split ? !(D < merge_thr) : D > split_thr;
 }
 
 // One warp: leaf level of the tile's 64 cells (2 per lane) from its mask, and the tile's
@@ -99,8 +120,8 @@ __device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y
 
 __global__ void __launch_bounds__(256)
 quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint32_t var_thr,
-                float corner_thr, uint32_t* __restrict__ tile_mask, uint8_t* __restrict__ cell_level,
-                uint32_t* __restrict__ hist)
+                float corner_thr, QtTemporal tq, uint32_t* __restrict__ tile_mask,
+                uint8_t* __restrict__ cell_level, uint32_t* __restrict__ hist)
 {
     __shared__ Moments cell[64];          // 8x8 cells, index cy*8 + cx
     __shared__ Moments node2[16];         // level-2 nodes (16x16 pixels), index 4c + g
@@ -157,6 +178,8 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
     // Lane t < 21 owns node t: 0 root, 1..4 level 1 (c = t-1), 5..20 level 2 (c = (t-5)>>2,
     // g = (t-5)&3) -- the same numbering as the mask bits.
     bool flag = false;
+    const uint32_t prev = tq.prev_mask ? tq.prev_mask[tile] : 0u;
+    const bool was_split = lane < 21 && ((prev >> lane) & 1u);   // lane t = node t = mask bit t
     if (metric == NOIT_QT_VARIANCE) {
         Moments m = {0, {0, 0, 0}, {0, 0, 0}};
         if (lane >= 5 && lane < 21) {                    // level 2: 2x2 cells
@@ -191,7 +214,7 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
                 for (int k = 0; k < 3; ++k) { m.s1[k] += q.s1[k]; m.s2[k] += q.s2[k]; }
             }
         }
-        flag = lane < 21 && variance_splits(m, var_thr);
+        flag = lane < 21 && variance_splits(m, var_thr, tq.var_merge, was_split);
     } else if (lane < 21) {
         int x0 = X, y0 = Y, side = 64;
         if (lane >= 5) {
@@ -201,7 +224,7 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
             const int c = lane - 1;
             x0 = X + 32 * (c & 1); y0 = Y + 32 * (c >> 1); side = 32;
         }
-        flag = corner_splits(image, W, H, x0, y0, side, corner_thr);
+        flag = corner_splits(image, W, H, x0, y0, side, corner_thr, tq.corner_merge, was_split);
     }
     // top-down: a node's flag counts only if its parent split
     const uint32_t F = __ballot_sync(0xffffffffu, flag);
@@ -212,8 +235,61 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
         for (int c = 0; c < 4; ++c)
             if ((F >> (1 + c)) & 1u) mask |= (1u << (1 + c)) | (F & (0xFu << (5 + 4 * c)));
     }
+    if (tq.prev_mask && tq.max_step > 0) {               // at most max_step levels per frame
+        const int pd = mask_depth(prev), d = mask_depth(mask);
+        if (d > pd + tq.max_step) {                      // truncate below depth pd + max_step
+            const int lim = pd + tq.max_step;
+            mask &= lim == 0 ? 0u : (lim == 1 ? 0x1u : (lim == 2 ? 0x1Fu : 0x1FFFFFu));
+        } else if (d < pd - tq.max_step) {               // refine uniformly to depth pd - max_step
+            const int lim = pd - tq.max_step;
+            mask |= (lim >= 1 ? 1u : 0u) | (lim >= 2 ? 0x1Eu : 0u) | (lim >= 3 ? 0x1FFFE0u : 0u);
+        }
+    }
     if (tile_mask && lane == 0) tile_mask[tile] = mask;
     emit_levels_and_hist(mask, X, Y, W, H, lane, cell_level, hist);
+}
+
+static noit_status quadtree_launch(noit_ctx* ctx, const char* who, const float* image, int32_t width,
+                                   int32_t height, int32_t metric, uint32_t var_thr, float corner_thr,
+                                   QtTemporal tq, uint32_t* tile_mask, uint8_t* cell_level,
+                                   uint32_t* level_hist, void* stream)
+{
+    if (!tile_mask && !cell_level && !level_hist)
+        return noit_fail(ctx, NOIT_ERR_NULL, "%s: every output is NULL", who);
+    if (width <= 0 || height <= 0 || (uint64_t)width * (uint64_t)height + 1 > 0xFFFFFFFFull)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "%s: bad width/height", who);
+    if (metric != NOIT_QT_VARIANCE && metric != NOIT_QT_CORNER)
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: unknown metric %d", who, metric);
+    if (!noit_aligned(image, 16))
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: image needs 16-byte alignment", who);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
+    const int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
+    quadtree_kernel<<<Tx * Ty, 256, 0, st>>>(image, width, height, metric, var_thr, corner_thr, tq,
+                                             tile_mask, cell_level, level_hist);
+    ctx->launches += 1;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    return NOIT_OK;
+}
+
+extern "C" noit_status noit_quadtree_temporal(noit_ctx* ctx, const float* image, int32_t width,
+                                              int32_t height, const noit_qt_temporal_params* params,
+                                              const uint32_t* prev_tile_mask, uint32_t* tile_mask,
+                                              uint8_t* cell_level, uint32_t* level_hist, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree_temporal: ctx is NULL");
+    if (!image || !params)
+        return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_temporal: image/params is NULL");
+    if (params->max_level_step < 0 || params->max_level_step > 3)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_temporal: max_level_step must be in [0, 3]");
+    if (params->var_merge_q > params->var_split_q || params->corner_merge > params->corner_split)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_temporal: merge threshold above split threshold");
+    if (prev_tile_mask && prev_tile_mask == tile_mask)
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree_temporal: prev_tile_mask aliases tile_mask");
+    QtTemporal tq = {prev_tile_mask, params->var_merge_q, params->corner_merge, params->max_level_step};
+    return quadtree_launch(ctx, "noit_quadtree_temporal", image, width, height, params->metric,
+                           params->var_split_q, params->corner_split, tq, tile_mask, cell_level,
+                           level_hist, stream);
 }
 
 extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t width, int32_t height,
@@ -222,35 +298,15 @@ extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t 
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree: ctx is NULL");
     if (!image || !params) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree: image/params is NULL");
-    if (!tile_mask && !cell_level && !level_hist)
-        return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree: every output is NULL");
-    if (width <= 0 || height <= 0 || (uint64_t)width * (uint64_t)height + 1 > 0xFFFFFFFFull)
-        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree: bad width/height");
-    if (params->metric != NOIT_QT_VARIANCE && params->metric != NOIT_QT_CORNER)
-        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree: unknown metric %d", params->metric);
-    if (!noit_aligned(image, 16))
-        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree: image needs 16-byte alignment");
-    cudaStream_t st = (cudaStream_t)stream;
-    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
-    const int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
-    quadtree_kernel<<<Tx * Ty, 256, 0, st>>>(image, width, height, params->metric,
-                                             params->var_threshold_q, params->corner_threshold,
-                                             tile_mask, cell_level, level_hist);
-    ctx->launches += 1;
-    NOIT_CUDA(ctx, cudaGetLastError());
-    return NOIT_OK;
+    QtTemporal tq = {nullptr, 0u, 0.f, 0};
+    return quadtree_launch(ctx, "noit_quadtree", image, width, height, params->metric,
+                           params->var_threshold_q, params->corner_threshold, tq, tile_mask, cell_level,
+                           level_hist, stream);
 }
 
 // ------------------------------------------------------------------------------------------
 // NEXT-1: quadtree consistency + demand index (O10, reading A25)
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ int mask_depth(uint32_t mask)
-{
-    if (!(mask & 1u)) return 0;
-    if (!(mask & 0x1Eu)) return 1;
-    return (mask & 0x1FFFE0u) ? 3 : 2;
-}
-
 __global__ void __launch_bounds__(256)
 tile_depth_kernel(const uint32_t* __restrict__ tile_mask, int n, uint8_t* __restrict__ depth)
 {

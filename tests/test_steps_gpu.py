@@ -358,6 +358,49 @@ def test_quadtree_then_balance_on_cfg4(noit, cfg4_small):
     assert np.max(np.abs(got["scales"].cpu().numpy() - ref["scales"])) <= 1e-6
 
 
+# -------------------------------------------------------------------------------------------
+# NEXT-2: temporal tile state (O11)
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,W,H,metric,step,hist_", [(0, 520, 330, 0, 1, True), (1, 520, 330, 1, 1, True),
+                                                        (2, 1920, 1080, 0, 1, True), (3, 200, 136, 0, 0, True),
+                                                        (4, 200, 136, 1, 2, True), (5, 64, 64, 0, 1, False)])
+def test_quadtree_temporal_random(noit, seed, W, H, metric, step, hist_):
+    from test_oracle_pins import _random_valid_masks
+    rng = np.random.default_rng(100 + seed)
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    img = (rng.random((H * W, 4)) * rng.random((H * W, 1)) ** 3).astype(np.float32)
+    yy = np.arange(H * W) // W
+    img[yy < H // 3] = 0.25                                                    # a flat band: merges
+    prev = _random_valid_masks(rng, Tx * Ty) if hist_ else None
+    kw = dict(metric=metric, var_split=2500, var_merge=1500, corner_split=0.35, corner_merge=0.2,
+              max_step=step)
+    ref = oracle.quadtree_temporal(img, W, H, prev, **kw)
+    ctx = noit.Noit()
+    d_prev = None if prev is None else torch.from_numpy(prev.view(np.int32).copy()).cuda()
+    got = ctx.quadtree_temporal(torch.from_numpy(img).cuda(), W, H, d_prev, **kw)
+    qt_equal(got, ref)
+    if prev is not None:
+        assert not np.array_equal(ref["tile_mask"], oracle.quadtree_temporal(img, W, H, None, **kw)["tile_mask"])
+
+
+def test_quadtree_temporal_chain_over_cfg5_frames(noit):
+    """Tiles of frame t steer frame t+1: four frames of the reduced cfg5 sequence."""
+    seq = noit_scenes.cfg5(0, W=960, H=540)
+    ctx = noit.Noit(seq.weights, seq.mlp_precision)
+    W, H = seq.width, seq.height
+    g_prev = r_prev = None
+    depths = []
+    for t in range(4):
+        fb = noit.DeviceFragBuf.from_host(seq.frame(t))
+        img = ctx.resolve(fb, seq.background, want=("final",))["final"]
+        got = ctx.quadtree_temporal(img, W, H, g_prev, var_split=6, var_merge=3, max_step=1)
+        ref = oracle.quadtree_temporal(img.cpu().numpy(), W, H, r_prev, var_split=6, var_merge=3, max_step=1)
+        qt_equal(got, ref)
+        g_prev, r_prev = got["tile_mask"], ref["tile_mask"]
+        depths.append(ref["hist"].tolist())
+    assert depths[0] != depths[1]                                              # the history matters
+
+
 def test_abi_errors(noit, cfg1_scene):
     import ctypes as C
     sc = cfg1_scene
