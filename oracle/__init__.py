@@ -145,6 +145,22 @@ def quadtree(image: np.ndarray, width: int, height: int, metric: int = 0,
     return out
 
 
+def quadtree16(image: np.ndarray, width: int, height: int, metric: int = 1,
+               var_threshold_q: int = 6, corner_threshold: float = 0.02) -> dict:
+    """O6 in the paper's own geometry: 16x16 base tiles down to 2x2 leaves."""
+    img = _chk(np.ascontiguousarray(image, np.float32), np.float32, width * height * 4)
+    Tx, Ty = (width + 15) // 16, (height + 15) // 16
+    cx, cy = (width + 1) // 2, (height + 1) // 2
+    out = dict(tile_mask=np.zeros(Tx * Ty, np.uint32), cell_level=np.zeros(cx * cy, np.uint8),
+               hist=np.zeros(4, np.uint32))
+    rc = lib().oracle_quadtree_base(_p(img), C.c_int32(width), C.c_int32(height), C.c_int32(metric),
+                                    C.c_uint32(var_threshold_q), C.c_float(corner_threshold),
+                                    C.c_int32(16), _p(out["tile_mask"]), _p(out["cell_level"]),
+                                    _p(out["hist"]))
+    assert rc == 0
+    return out
+
+
 def quadtree_balance(tile_mask: np.ndarray, width: int, height: int, iterations: int = 2,
                      delta2: float = 2.2, delta3: float = 3.0) -> dict:
     """O10: 2:1 tile balance by Jacobi relaxation + histogram + demand index and Eq. 2 scales."""

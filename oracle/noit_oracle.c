@@ -458,64 +458,76 @@ static int node_splits(const qt_args *a, int x0, int y0, int side)
  * Mask bits: 0 = root split; 1+c = level-1 child c split (c = cx + 2cy); 5+4c+g = level-2
  * grandchild g of child c split (g = gx + 2gy).  Top-down: a node is evaluated only if its
  * parent split.  Level-3 nodes (8x8) never split.                                      */
-int32_t oracle_quadtree(const float *image, int32_t width, int32_t height, int32_t metric,
-                        uint32_t var_threshold_q, float corner_threshold, uint32_t *tile_mask,
-                        uint8_t *cell_level, uint32_t *hist)
+/* Generic in the base tile side B (64: BASELINE.json's sizes, 16: the paper's own 16 -> 2,     */
+/* P:61): node sides B, B/2, B/4, leaves down to B/8; cells are B/8 square. */
+int32_t oracle_quadtree_base(const float *image, int32_t width, int32_t height, int32_t metric,
+                             uint32_t var_threshold_q, float corner_threshold, int32_t base,
+                             uint32_t *tile_mask, uint8_t *cell_level, uint32_t *hist)
 {
+    if (base != 64 && base != 16) return 1;
     qt_args a = {image, width, height, metric, var_threshold_q, corner_threshold};
-    int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
-    int cells_x = (width + 7) / 8, cells_y = (height + 7) / 8;
+    const int B = base, cs = base / 8;                   /* cell side */
+    int Tx = (width + B - 1) / B, Ty = (height + B - 1) / B;
+    int cells_x = (width + cs - 1) / cs, cells_y = (height + cs - 1) / cs;
     uint64_t h[4] = {0, 0, 0, 0};
     for (int ty = 0; ty < Ty; ++ty)
         for (int tx = 0; tx < Tx; ++tx) {
-            int X = tx * 64, Y = ty * 64;
+            int X = tx * B, Y = ty * B;
             uint32_t mask = 0;
-            uint8_t lvl[8][8];                       /* leaf level of each 8x8 cell of the tile */
+            uint8_t lvl[8][8];                       /* leaf level of each cell of the tile */
             memset(lvl, 0, sizeof lvl);
-            if (node_splits(&a, X, Y, 64)) {
+            if (node_splits(&a, X, Y, B)) {
                 mask |= 1u;
                 for (int c = 0; c < 4; ++c) {
-                    int cx = X + 32 * (c & 1), cy = Y + 32 * (c >> 1);
-                    int child_split = node_splits(&a, cx, cy, 32);
+                    int cx = X + (B / 2) * (c & 1), cy = Y + (B / 2) * (c >> 1);
+                    int child_split = node_splits(&a, cx, cy, B / 2);
                     if (child_split) mask |= 1u << (1 + c);
                     for (int g = 0; g < 4; ++g) {
-                        int gx = cx + 16 * (g & 1), gy = cy + 16 * (g >> 1);
+                        int gx = cx + (B / 4) * (g & 1), gy = cy + (B / 4) * (g >> 1);
                         int level = 1;
                         if (child_split) {
                             level = 2;
-                            if (node_splits(&a, gx, gy, 16)) {
+                            if (node_splits(&a, gx, gy, B / 4)) {
                                 mask |= 1u << (5 + 4 * c + g);
                                 level = 3;
                             }
                         }
                         for (int v = 0; v < 2; ++v)
                             for (int u = 0; u < 2; ++u)
-                                lvl[(gy - Y) / 8 + v][(gx - X) / 8 + u] = (uint8_t)level;
+                                lvl[(gy - Y) / cs + v][(gx - X) / cs + u] = (uint8_t)level;
                     }
                 }
             }
             if (tile_mask) tile_mask[ty * Tx + tx] = mask;
             /* histogram: leaves that contain >= 1 in-image pixel, counted once each           */
             for (int level = 0; level < 4; ++level) {
-                int side = 64 >> level, per = 1 << level;
+                int side = B >> level, per = 1 << level;
                 for (int ny = 0; ny < per; ++ny)
                     for (int nx = 0; nx < per; ++nx) {
                         int x0 = X + nx * side, y0 = Y + ny * side;
                         if (x0 >= width || y0 >= height) continue;
-                        if (lvl[(y0 - Y) / 8][(x0 - X) / 8] != level) continue;
+                        if (lvl[(y0 - Y) / cs][(x0 - X) / cs] != level) continue;
                         /* a leaf at `level` is the node whose own level equals the cell's    */
                         h[level] += 1;
                     }
             }
             for (int v = 0; v < 8; ++v)
                 for (int u = 0; u < 8; ++u) {
-                    int cxg = X / 8 + u, cyg = Y / 8 + v;
+                    int cxg = X / cs + u, cyg = Y / cs + v;
                     if (cxg < cells_x && cyg < cells_y && cell_level)
                         cell_level[cyg * cells_x + cxg] = lvl[v][u];
                 }
         }
     if (hist) for (int k = 0; k < 4; ++k) hist[k] = (uint32_t)h[k];
     return 0;
+}
+
+int32_t oracle_quadtree(const float *image, int32_t width, int32_t height, int32_t metric,
+                        uint32_t var_threshold_q, float corner_threshold, uint32_t *tile_mask,
+                        uint8_t *cell_level, uint32_t *hist)
+{
+    return oracle_quadtree_base(image, width, height, metric, var_threshold_q, corner_threshold, 64,
+                                tile_mask, cell_level, hist);
 }
 
 /* ---------------------------------------------------------------------------------------- */

@@ -816,3 +816,33 @@ def test_temporal_step_limit_and_mask_validity_random():
             for g in range(4):
                 if b >> (5 + 4 * c + g) & 1:
                     assert b >> (1 + c) & 1
+
+
+# -------------------------------------------------------------------------------------------
+# NEXT-3: the paper's own tile geometry, 16x16 base tiles down to 2x2
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("metric,W,H", [(0, 48, 32), (1, 48, 32), (0, 37, 21), (1, 37, 21)])
+def test_quadtree16_equals_quadtree64_of_the_4x_replicated_image(metric, W, H):
+    """Replicating every pixel 4x4 maps a 16-tile onto a 64-tile: the variance terms scale by the
+    same factor on both sides of the test (n S2 - S1^2 and n^2 both by 256) and the corner pixels
+    are the same pixels, so every decision, cell level and leaf count must coincide."""
+    rng = np.random.default_rng(50 + metric)
+    img = (rng.random((H, W, 4)) * rng.random((H, W, 1)) ** 2).astype(np.float32)
+    img[: H // 3] = 0.4
+    big = np.repeat(np.repeat(img, 4, axis=0), 4, axis=1)
+    a = oracle.quadtree16(img.reshape(-1, 4), W, H, metric, 900, 0.2)
+    b = oracle.quadtree(big.reshape(-1, 4), 4 * W, 4 * H, metric, 900, 0.2)
+    assert len(set(a["tile_mask"].tolist())) > 1                 # not a degenerate forest
+    for k in ("tile_mask", "cell_level", "hist"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_quadtree16_constant_and_checkerboard():
+    W, H = 64, 48
+    r = oracle.quadtree16(np.full((H * W, 4), 0.3, np.float32), W, H, 1)
+    assert not r["tile_mask"].any() and r["hist"].tolist() == [12, 0, 0, 0]
+    yy, xx = np.mgrid[0:H, 0:W]
+    img = np.zeros((H, W, 4), np.float32)
+    img[..., :3] = ((xx + yy) & 1)[..., None]
+    r = oracle.quadtree16(img.reshape(-1, 4), W, H, 0, 6)
+    assert np.all(r["tile_mask"] == 0x1FFFFF) and r["hist"].tolist() == [0, 0, 0, 12 * 64]
