@@ -158,6 +158,14 @@ noit_status noit_quadtree(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t 
                           int32_t height, const noit_qt_params* params, uint32_t* tile_mask,
                           uint8_t* cell_level, uint32_t* level_hist, void* stream);
 
+/* ---- NEXT-3: noit_quadtree in the paper's own geometry: 16x16 base tiles, four levels
+ * down to 2x2 leaves; same metrics, mask layout and top-down rule.
+ *   tile_mask [ceil(H/16)*ceil(W/16)], cell_level [ceil(H/2)*ceil(W/2)] (leaf level of every 2x2
+ *   cell), level_hist [4] (zeroed by the call).                                              */
+noit_status noit_quadtree16(noit_ctx* ctx, const float* image /*[P][4]*/, int32_t width,
+                            int32_t height, const noit_qt_params* params, uint32_t* tile_mask,
+                            uint8_t* cell_level, uint32_t* level_hist, void* stream);
+
 /* ---- NEXT-2: temporal tile state ("tiles computed in frame F_t guide ... F_t+1", P:61
  * split / merge thresholds, "tiles may change by only one level per frame"; O11, A26).
  * noit_quadtree with a memory: a node that was NOT split in prev_tile_mask splits iff

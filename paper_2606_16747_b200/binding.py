@@ -22,7 +22,7 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
-           "noit_quadtree_balance",
+           "noit_quadtree_balance", "noit_quadtree16",
            "noit_reproject"]
 
 
@@ -272,6 +272,24 @@ class Noit:
         self._check(self._L.noit_quadtree(self._ctx, _ptr(image), C.c_int32(width), C.c_int32(height),
                                           C.byref(prm), _ptr(out["tile_mask"]), _ptr(out["cell_level"]),
                                           _ptr(out["hist"]), _stream(stream)))
+        return out
+
+    # ---- NEXT-3 -----------------------------------------------------------------------
+    def quadtree16(self, image: torch.Tensor, width: int, height: int, metric: int = QT_CORNER,
+                   var_threshold_q: int = 6, corner_threshold: float = 0.02, out=None, stream=None):
+        """The paper's tile geometry: 16x16 base tiles down to 2x2 leaves."""
+        assert image.dtype == torch.float32 and image.is_contiguous()
+        dev = image.device
+        Tx, Ty = (width + 15) // 16, (height + 15) // 16
+        cx, cy = (width + 1) // 2, (height + 1) // 2
+        if out is None:
+            out = dict(tile_mask=torch.empty(Tx * Ty, dtype=torch.int32, device=dev),
+                       cell_level=torch.empty(cx * cy, dtype=torch.uint8, device=dev),
+                       hist=torch.empty(4, dtype=torch.int32, device=dev))
+        prm = QtParamsC(metric, var_threshold_q, corner_threshold)
+        self._check(self._L.noit_quadtree16(self._ctx, _ptr(image), C.c_int32(width), C.c_int32(height),
+                                            C.byref(prm), _ptr(out["tile_mask"]), _ptr(out["cell_level"]),
+                                            _ptr(out["hist"]), _stream(stream)))
         return out
 
     # ---- NEXT-2 -----------------------------------------------------------------------

@@ -74,6 +74,7 @@ __device__ bool corner_splits(const float* __restrict__ image, int W, int H, int
 // One warp: leaf level of the tile's 64 cells (2 per lane) from its mask, and the tile's
 // contribution to the histogram of leaves that hold >= 1 in-image pixel (a leaf at level l is
 // the node whose first cell has level l).  Shared by noit_quadtree and noit_quadtree_balance.
+template <int kCellShift>                               // cell side = 1 << kCellShift pixels (8 or 2)
 __device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y, int W, int H, int lane,
                                                      uint8_t* __restrict__ cell_level,
                                                      uint32_t* __restrict__ hist)
@@ -84,13 +85,14 @@ __device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y
         if (!((mask >> (1 + c)) & 1u)) return 1;
         return ((mask >> (5 + 4 * c + g)) & 1u) ? 3 : 2;
     };
-    const int cells_w = (W + 7) >> 3, cells_h = (H + 7) >> 3;
+    constexpr int kCell = 1 << kCellShift;
+    const int cells_w = (W + kCell - 1) >> kCellShift, cells_h = (H + kCell - 1) >> kCellShift;
     uint32_t h3 = 0;
 #pragma unroll
     for (int k = 0; k < 2; ++k) {                        // 64 cells, 2 per lane
         const int idx = lane + 32 * k, cx = idx & 7, cy = idx >> 3;
         const int level = level_of_cell(cx, cy);
-        const int gx = (X >> 3) + cx, gy = (Y >> 3) + cy;
+        const int gx = (X >> kCellShift) + cx, gy = (Y >> kCellShift) + cy;
         const bool in_image = gx < cells_w && gy < cells_h;
         if (cell_level && in_image) cell_level[(size_t)gy * cells_w + gx] = (uint8_t)level;
         h3 += __popc(__ballot_sync(0xffffffffu, in_image && level == 3));
@@ -106,7 +108,7 @@ __device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y
         } else if (lane >= 1) {
             cx = 4 * ((lane - 1) & 1); cy = 4 * ((lane - 1) >> 1); lv = 1;
         }
-        leaf = X + 8 * cx < W && Y + 8 * cy < H && level_of_cell(cx, cy) == lv;
+        leaf = X + kCell * cx < W && Y + kCell * cy < H && level_of_cell(cx, cy) == lv;
     }
     const uint32_t Lf = __ballot_sync(0xffffffffu, leaf);
     if (lane == 0) {
@@ -246,7 +248,7 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
         }
     }
     if (tile_mask && lane == 0) tile_mask[tile] = mask;
-    emit_levels_and_hist(mask, X, Y, W, H, lane, cell_level, hist);
+    emit_levels_and_hist<3>(mask, X, Y, W, H, lane, cell_level, hist);
 }
 
 static noit_status quadtree_launch(noit_ctx* ctx, const char* who, const float* image, int32_t width,
@@ -351,7 +353,7 @@ balance_kernel(const uint8_t* __restrict__ depth0, int W, int H, int Tx, int Ty,
             tile_mask[tile] = mask;
             if (tile_level) tile_level[tile] = (uint8_t)best;
         }
-        emit_levels_and_hist(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist);
+        emit_levels_and_hist<3>(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist);
     }
     if (!scales) return;
     // last block: demand index and Eq. 2
@@ -407,6 +409,132 @@ extern "C" noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32
                                                 delta2, delta3, tile_mask, tile_level, cell_level,
                                                 level_hist, scales, ctx->d_counters + 2);
     ctx->launches += 2;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    return NOIT_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// NEXT-3: the paper's own tile geometry: 16x16 base tiles, four levels down to 2x2
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ Moments moments_xor_add(const Moments& m, int lane_mask)
+{
+    Moments r;
+    r.n = m.n + __shfl_xor_sync(0xffffffffu, m.n, lane_mask);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        r.s1[k] = m.s1[k] + __shfl_xor_sync(0xffffffffu, m.s1[k], lane_mask);
+        r.s2[k] = m.s2[k] + __shfl_xor_sync(0xffffffffu, m.s2[k], lane_mask);
+    }
+    return r;
+}
+
+// One WARP per 16x16 tile (a tile is 4 KB: a CTA per tile would be all latency).  The tile's 64
+// cells are 2x2 pixels; lane l holds cells (cx, cy) = (l & 7, l >> 3) and (cx, cy + 4), so the
+// sums of a level-2 node (2x2 cells) are a butterfly over lane bits 0 and 3, of a level-1 node
+// additionally over bits 1 and 4, of the root over bit 2 plus the lane's two halves.  Every lane
+// then knows the split flag of each node it belongs to; lane t < 21 picks node t's flag from the
+// ballot of a representative lane, and the mask is assembled exactly as in quadtree_kernel.
+__global__ void __launch_bounds__(128)
+quadtree16_kernel(const float* __restrict__ image, int W, int H, int metric, uint32_t var_thr,
+                  float corner_thr, uint32_t* __restrict__ tile_mask, uint8_t* __restrict__ cell_level,
+                  uint32_t* __restrict__ hist)
+{
+    const int Tx = (W + 15) >> 4, Ty = (H + 15) >> 4;
+    const int tile = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (tile >= Tx * Ty) return;
+    const int tx = tile % Tx, ty = tile / Tx, X = tx << 4, Y = ty << 4;
+    bool flag = false;
+    if (metric == NOIT_QT_VARIANCE) {
+        Moments half[2];
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {
+            Moments m = {0, {0, 0, 0}, {0, 0, 0}};
+            const int cx = lane & 7, cy = (lane >> 3) + 4 * hb;
+#pragma unroll
+            for (int v = 0; v < 2; ++v) {
+                const int y = Y + 2 * cy + v, x = X + 2 * cx;
+                if (y >= H) continue;
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    if (x + u >= W) continue;
+                    const float4 px = __ldcs(reinterpret_cast<const float4*>(image) + (size_t)y * W + x + u);
+                    const uint32_t q[3] = {quant8(px.x), quant8(px.y), quant8(px.z)};
+                    m.n += 1;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { m.s1[k] += q[k]; m.s2[k] += q[k] * q[k]; }
+                }
+            }
+            half[hb] = m;
+        }
+        Moments n2[2], n1[2];
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {
+            n2[hb] = moments_xor_add(moments_xor_add(half[hb], 1), 8);    // 2x2 cells
+            n1[hb] = moments_xor_add(moments_xor_add(n2[hb], 2), 16);     // 4x4 cells
+        }
+        Moments root = n1[0];
+        root.n += n1[1].n;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { root.s1[k] += n1[1].s1[k]; root.s2[k] += n1[1].s2[k]; }
+        root = moments_xor_add(root, 4);
+        const uint32_t F0 = __ballot_sync(0xffffffffu, variance_splits(root, var_thr, 0u, false));
+        const uint32_t F1[2] = {__ballot_sync(0xffffffffu, variance_splits(n1[0], var_thr, 0u, false)),
+                                __ballot_sync(0xffffffffu, variance_splits(n1[1], var_thr, 0u, false))};
+        const uint32_t F2[2] = {__ballot_sync(0xffffffffu, variance_splits(n2[0], var_thr, 0u, false)),
+                                __ballot_sync(0xffffffffu, variance_splits(n2[1], var_thr, 0u, false))};
+        if (lane == 0) {
+            flag = F0 & 1u;
+        } else if (lane < 5) {                           // child c: cells (4(c&1).., 4(c>>1)..)
+            const int c = lane - 1;
+            flag = (F1[c >> 1] >> (4 * (c & 1))) & 1u;
+        } else if (lane < 21) {                          // grandchild g of child c
+            const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+            flag = (F2[c >> 1] >> (16 * (g >> 1) + 4 * (c & 1) + 2 * (g & 1))) & 1u;
+        }
+    } else if (lane < 21) {
+        int x0 = X, y0 = Y, side = 16;
+        if (lane >= 5) {
+            const int c = (lane - 5) >> 2, g = (lane - 5) & 3;
+            x0 = X + 8 * (c & 1) + 4 * (g & 1); y0 = Y + 8 * (c >> 1) + 4 * (g >> 1); side = 4;
+        } else if (lane >= 1) {
+            const int c = lane - 1;
+            x0 = X + 8 * (c & 1); y0 = Y + 8 * (c >> 1); side = 8;
+        }
+        flag = corner_splits(image, W, H, x0, y0, side, corner_thr, 0.f, false);
+    }
+    const uint32_t F = __ballot_sync(0xffffffffu, flag);    // top-down gating
+    uint32_t mask = 0;
+    if (F & 1u) {
+        mask = 1u;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if ((F >> (1 + c)) & 1u) mask |= (1u << (1 + c)) | (F & (0xFu << (5 + 4 * c)));
+    }
+    if (tile_mask && lane == 0) tile_mask[tile] = mask;
+    emit_levels_and_hist<1>(mask, X, Y, W, H, lane, cell_level, hist);
+}
+
+extern "C" noit_status noit_quadtree16(noit_ctx* ctx, const float* image, int32_t width, int32_t height,
+                                       const noit_qt_params* params, uint32_t* tile_mask,
+                                       uint8_t* cell_level, uint32_t* level_hist, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree16: ctx is NULL");
+    if (!image || !params) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree16: image/params is NULL");
+    if (!tile_mask && !cell_level && !level_hist)
+        return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree16: every output is NULL");
+    if (width <= 0 || height <= 0 || (uint64_t)width * (uint64_t)height + 1 > 0xFFFFFFFFull)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree16: bad width/height");
+    if (params->metric != NOIT_QT_VARIANCE && params->metric != NOIT_QT_CORNER)
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree16: unknown metric %d", params->metric);
+    if (!noit_aligned(image, 16))
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree16: image needs 16-byte alignment");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
+    const int tiles = ((width + 15) / 16) * ((height + 15) / 16);
+    quadtree16_kernel<<<(tiles + 3) / 4, 128, 0, st>>>(image, width, height, params->metric,
+                                                       params->var_threshold_q, params->corner_threshold,
+                                                       tile_mask, cell_level, level_hist);
+    ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
 }

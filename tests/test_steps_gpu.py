@@ -401,6 +401,22 @@ def test_quadtree_temporal_chain_over_cfg5_frames(noit):
     assert depths[0] != depths[1]                                              # the history matters
 
 
+# -------------------------------------------------------------------------------------------
+# NEXT-3: the paper's tile geometry, 16x16 -> 2x2
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed,W,H,metric", [(0, 1920, 1080, 1), (1, 1920, 1080, 0), (2, 37, 21, 0),
+                                             (3, 37, 21, 1), (4, 333, 130, 0), (5, 16, 16, 1)])
+def test_quadtree16_random_images(noit, seed, W, H, metric):
+    rng = np.random.default_rng(200 + seed)
+    img = (rng.random((H * W, 4)) * rng.random((H * W, 1)) ** 2).astype(np.float32)
+    yy = np.arange(H * W) // W
+    img[yy < H // 3] = 0.4
+    ref = oracle.quadtree16(img, W, H, metric, 900, 0.2)
+    got = noit.Noit().quadtree16(torch.from_numpy(img).cuda(), W, H, metric, 900, 0.2)
+    qt_equal(got, ref)
+    assert len(set(ref["tile_mask"].tolist())) > 1 or W * H <= 256
+
+
 def test_abi_errors(noit, cfg1_scene):
     import ctypes as C
     sc = cfg1_scene
