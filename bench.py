@@ -294,6 +294,25 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     e2e_ms = max_over_ranks(dist, e0.elapsed_time(e1) / e2e_steps, dev)
+    # entry points outside the step (NEXT-2, NEXT-3): CUDA-event means, reported as `extras_ms`
+    def timed(fn, n=20):
+        for _ in range(3):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+    tq = {"o": None}
+    q16 = {"o": None}
+    def run_temporal():
+        tq["o"] = ctx.quadtree_temporal(plain["final"], W, H, qt["tile_mask"], out=tq["o"])
+    def run_q16():
+        q16["o"] = ctx.quadtree16(plain["final"], W, H, noit.QT_CORNER, 6, 0.02, out=q16["o"])
+    extras = {"quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
+              "quadtree_balance": timed(lambda: ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal))}
     clocks = sampler.stop() if rank == 0 else None
     rejected = int(rp["reject_count"].item())
     hist = bal["hist"].cpu().numpy().view(np.uint32).tolist()
@@ -313,7 +332,7 @@ def run_ours(args):
                        "l2": "inputs (647 MB) larger than L2 (126 MB); no flush", "seed": "rank"},
             "resolve_mpix_s": P * world / (resolve_ms * 1e-3) / 1e6,
             "resolve_gfrag_s": F * world / (resolve_ms * 1e-3) / 1e9,
-            "kernel_ms": per_kernel,
+            "kernel_ms": per_kernel, "extras_ms": extras,
             "roofline": {"bound": "hbm", "kernel": "noit_resolve (plain fused, S1-S5)", "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                          "algorithmic_bytes": rbytes, "traffic": resolve_traffic(),
