@@ -120,6 +120,28 @@ def resolve(fb, weights_eff, background, half=None, quarter=None, cell_level=Non
     return out
 
 
+def snap_lod(scale) -> int:
+    """Reading A27: power-of-two snap of an Eq. 2 scale (fp32 compare): 0 = full, 1 = half,
+    2 = quarter resolution."""
+    s = np.float32(scale)
+    return 0 if s > np.float32(0.70710678) else (1 if s > np.float32(0.35355339) else 2)
+
+
+def resolve_global(fb, half, quarter, weights_eff, background, lod2: int, lod3: int) -> dict:
+    """O7g: layer 1 at full resolution, pass 2 (layer 2) at lod2 and pass 3 (tail) at lod3 for the
+    whole frame, bilinear upsampling, features / MLP / composite at full resolution."""
+    P = fb.width * fb.height
+    out = dict(trans=np.zeros((P, 4), np.float32), final=np.zeros((P, 4), np.float32),
+               depth1=np.zeros(P, np.float32))
+    bg = np.asarray(background, np.float32)
+    args = _fb_args(fb) + [C.c_int32(fb.color_fmt)] + _fb_args(half) + _fb_args(quarter)
+    args += [C.c_int32(lod2), C.c_int32(lod3), _p(_chk(weights_eff, np.float32, 771)), _p(bg),
+             _p(out["trans"]), _p(out["final"]), _p(out["depth1"])]
+    rc = lib().oracle_resolve_global(*args)
+    assert rc == 0, rc
+    return out
+
+
 def exact(fb, background) -> dict:
     """O5x: full sort + Porter-Duff over (Eq. 1) + background; and the exact tail composite."""
     P = fb.width * fb.height

@@ -302,6 +302,75 @@ static void resolve_pixel_coarse(const frag_view *fb, const frag_view *cb, int r
     store_outputs(p, ct, t2 * G[8], bg, L.d1, out_trans, out_final, out_depth1);
 }
 
+/* bilinear sample of G at the full-res pixel centre, taps clamped to the image only            */
+static void sample_G_image(const frag_view *cb, int r, int x, int y, double G[10])
+{
+    double u = (x + 0.5) / r - 0.5, v = (y + 0.5) / r - 0.5;
+    int i0 = (int)floor(u), j0 = (int)floor(v);
+    double wx = u - i0, wy = v - j0;
+    int xa = clampi(i0, 0, cb->width - 1), xb = clampi(i0 + 1, 0, cb->width - 1);
+    int ya = clampi(j0, 0, cb->height - 1), yb = clampi(j0 + 1, 0, cb->height - 1);
+    double g00[10], g10[10], g01[10], g11[10];
+    coarse_G(cb, xa, ya, g00);
+    coarse_G(cb, xb, ya, g10);
+    coarse_G(cb, xa, yb, g01);
+    coarse_G(cb, xb, yb, g11);
+    for (int k = 0; k < 10; ++k) {               /* lerp x first, then y                      */
+        double top = g00[k] + wx * (g10[k] - g00[k]);
+        double bot = g01[k] + wx * (g11[k] - g01[k]);
+        G[k] = top + wy * (bot - top);
+    }
+}
+
+/* O7g frame-global resolution control as the paper does it:      */
+/* pass 1 (layer 1) always at full resolution; pass 2 (layer 2) at lod2 and pass 3 (tail */
+/* statistics and N) at lod3 for the WHOLE frame, lod_p = the power-of-two snap of the Eq. 2     */
+/* scale s_p (reading A27: lod 0 if s > 2^-0.5, 1 if s > 2^-1.5, else 2); lod 0 takes the        */
+/* pixel's own full-resolution list, lod > 0 the bilinear upsample of that pass's outputs from   */
+/* the half / quarter buffer, taps clamped to the image; features, MLP and composite at   */
+/* full resolution as in O7.                                                                     */
+int32_t oracle_resolve_global(int32_t width, int32_t height, const uint32_t *offsets, const float *depth,
+                              const void *rgba, int32_t color_fmt,
+                              int32_t hw, int32_t hh, const uint32_t *hoff, const float *hdepth,
+                              const void *hrgba,
+                              int32_t qw, int32_t qh, const uint32_t *qoff, const float *qdepth,
+                              const void *qrgba, int32_t lod2, int32_t lod3, const float *weights,
+                              const float *background, float *out_trans, float *out_final,
+                              float *out_depth1)
+{
+    frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
+    frag_view hb = {hw, hh, hoff, hdepth, hrgba, color_fmt};
+    frag_view qb = {qw, qh, qoff, qdepth, qrgba, color_fmt};
+    if (lod2 < 0 || lod2 > 2 || lod3 < 0 || lod3 > 2) return 2;
+    int64_t P = (int64_t)width * height;
+#pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t p = 0; p < P; ++p) {
+        int x = (int)(p % width), y = (int)(p / width);
+        pixel_layers L;
+        pixel_select_reduce(&fb, (size_t)p, &L);
+        double own[10], G2[10], G3[10];
+        for (int k = 0; k < 3; ++k) own[k] = L.c2[3] * L.c2[k];
+        own[3] = L.c2[3];
+        for (int k = 0; k < 3; ++k) own[4 + k] = L.c_acc[k];
+        own[7] = L.a_tail; own[8] = L.t_tail; own[9] = (double)L.n;
+        if (lod2 == 0) memcpy(G2, own, sizeof own);
+        else sample_G_image(lod2 == 1 ? &hb : &qb, 1 << lod2, x, y, G2);
+        if (lod3 == 0) memcpy(G3, own, sizeof own);
+        else if (lod3 == lod2) memcpy(G3, G2, sizeof G2);
+        else sample_G_image(lod3 == 1 ? &hb : &qb, 1 << lod3, x, y, G3);
+        float xf[5];
+        double f[3], ct[3];
+        int has_tail = features_from(G3[9], G3[8], &G3[4], G3[7], xf);
+        mlp_forward(weights, xf, f);
+        double a1 = L.c1[3];
+        double t2 = (1.0 - a1) * (1.0 - G2[3]);
+        for (int k = 0; k < 3; ++k)
+            ct[k] = a1 * L.c1[k] + (1.0 - a1) * G2[k] + (has_tail ? t2 * f[k] : 0.0);
+        store_outputs(p, ct, t2 * G3[8], background, L.d1, out_trans, out_final, out_depth1);
+    }
+    return 0;
+}
+
 /* S1-S5 (+S7 when cell_level != NULL, +S9 when pixel_list != NULL).
  * half/quarter buffers: pass width 0 to mark a buffer as absent.
  * cell_level[cy*ceil(W/8)+cx] in 0..3 ; level_to_lod[4] in {0,1,2}.

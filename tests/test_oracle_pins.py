@@ -846,3 +846,70 @@ def test_quadtree16_constant_and_checkerboard():
     img[..., :3] = ((xx + yy) & 1)[..., None]
     r = oracle.quadtree16(img.reshape(-1, 4), W, H, 0, 6)
     assert np.all(r["tile_mask"] == 0x1FFFFF) and r["hist"].tolist() == [0, 0, 0, 12 * 64]
+
+
+# -------------------------------------------------------------------------------------------
+# O7g: frame-global pass-2 / pass-3 resolution from the Eq. 2 scales (NEXT-1)
+# -------------------------------------------------------------------------------------------
+def _uniform_fb(W, H, depth, rgba, dtype=np.float32):
+    """Every pixel holds the same fragment list."""
+    n, P = len(depth), W * H
+    return make_fb(np.full(P, n), np.tile(np.asarray(depth, np.float32), P),
+                   np.tile(np.asarray(rgba, dtype), (P, 1)), width=W, height=H)
+
+
+def test_snap_lod_fixed_points():
+    got = [oracle.snap_lod(s) for s in (1.0, 0.75, 0.7071069, 0.7071066, 0.5, 0.36, 0.35, 0.25)]
+    assert got == [0, 0, 0, 1, 1, 1, 2, 2]
+
+
+def test_global_lod_zero_is_the_plain_resolve():
+    rng = np.random.default_rng(60)
+    W, H = 20, 12
+    counts = rng.integers(0, 9, W * H)
+    F = int(counts.sum())
+    fb = make_fb(counts, rng.uniform(0.05, 0.95, F), rng.uniform(0, 1, (F, 4)).astype(np.float32), W, H)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(6), 0)
+    a = oracle.resolve(fb, w, (0.2, 0.3, 0.4))
+    b = oracle.resolve_global(fb, None, None, w, (0.2, 0.3, 0.4), 0, 0)
+    for k in ("trans", "final", "depth1"):
+        assert np.allclose(a[k], b[k], rtol=1e-6, atol=1e-7), k
+
+
+@pytest.mark.parametrize("lod2,lod3", [(1, 1), (1, 2), (2, 2), (0, 2), (0, 1), (2, 1)])
+def test_global_lod_on_a_uniform_scene_equals_the_plain_resolve(lod2, lod3):
+    """If every pixel of every buffer holds the same list, up-sampling is the identity
+    (a + w (b - a) = a), so any pair of pass resolutions reproduces the plain resolve."""
+    W, H = 21, 13
+    depth = [0.5, 0.2, 0.8, 0.35, 0.6]
+    rgba = [[.9, .1, .2, .5], [.2, .8, .1, .3], [.1, .2, .9, .7], [.5, .5, .1, .4], [.3, .9, .9, .2]]
+    full = _uniform_fb(W, H, depth, rgba)
+    half = _uniform_fb((W + 1) // 2, (H + 1) // 2, depth, rgba)
+    quarter = _uniform_fb((W + 3) // 4, (H + 3) // 4, depth, rgba)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(7), 0)
+    a = oracle.resolve(full, w, (0.2, 0.3, 0.4))
+    b = oracle.resolve_global(full, half, quarter, w, (0.2, 0.3, 0.4), lod2, lod3)
+    for k in ("trans", "final", "depth1"):
+        assert np.allclose(a[k], b[k], rtol=1e-6, atol=1e-7), k
+
+
+def test_global_lod_upsamples_an_affine_layer2_alpha_exactly():
+    """Two fragments per pixel, black: T_tot = (1-a1)(1-a2_up).  With a2 affine in the coarse x the
+    bilinear sample at the full-res pixel centre is that affine function at (x+0.5)/r - 0.5,
+    clamped to the first / last texel centre at the border."""
+    W, H, r = 32, 4, 2
+    cw, ch = W // r, H // r
+    a1 = 0.25
+    full = _uniform_fb(W, H, [0.2, 0.6], [[0, 0, 0, a1], [0, 0, 0, 0.9]])
+    a2c = 0.1 + 0.05 * np.arange(cw)                                    # per coarse column
+    depth = np.tile(np.asarray([0.2, 0.6], np.float32), cw * ch)
+    rgba = np.zeros((cw * ch * 2, 4), np.float32)
+    rgba[0::2, 3] = a1
+    rgba[1::2, 3] = np.tile(a2c, ch)
+    half = make_fb(np.full(cw * ch, 2), depth, rgba, cw, ch)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(8), 0)
+    out = oracle.resolve_global(full, half, None, w, (0, 0, 0), 1, 0)
+    u = np.clip((np.arange(W) + 0.5) / r - 0.5, 0, cw - 1)
+    want = (1 - a1) * (1 - (0.1 + 0.05 * u))
+    got = out["trans"].reshape(H, W, 4)[..., 3]
+    assert np.allclose(got, np.tile(want, (H, 1)), rtol=1e-6, atol=1e-7)
