@@ -118,7 +118,14 @@ noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* 
  * with taps clamped to the pixel's own leaf, then features, MLP and composite run at full
  * resolution (A18-A20).  A level that maps to lod k > 0 requires the matching buffer.
  * pixel_list/pixel_count (device): resolve only the listed pixels (count read on the device),
- * leave the others untouched; not combinable with cell_level.                                */
+ * leave the others untouched; not combinable with cell_level.
+ * Frame-global resolution control (NEXT-1, the paper's own scheme P:78-87; O7g, A27): when
+ * pass_scales (device, float[3] = {w, s_2, s_3} as written by noit_quadtree_balance) is set,
+ * pass 2 (layer 2) is taken at lod2 and pass 3 (tail statistics, N) at lod3 for the WHOLE
+ * frame, lod_p = 0 if s_p > 2^-0.5, 1 if s_p > 2^-1.5, else 2, decided on the device (no host
+ * round trip); lod 0 = the pixel's own full-resolution list, lod 1 / 2 = bilinear upsample from
+ * `half` / `quarter` (both required), taps clamped to the image.  Not combinable with
+ * cell_level or pixel_list.                                                                  */
 typedef struct {
     noit_fragbuf full;
     const noit_fragbuf* half;        /* NULL => no S7                                          */
@@ -129,6 +136,7 @@ typedef struct {
     const uint32_t* pixel_list;      /* [<= P] pixel indices, or NULL                          */
     const uint32_t* pixel_count;     /* device scalar: entries of pixel_list to process        */
     float* out_trans; float* out_final; float* out_depth1;
+    const float* pass_scales;        /* device {w, s_2, s_3}, or NULL                          */
 } noit_resolve_desc;
 noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* desc, void* stream);
 

@@ -28,9 +28,11 @@ coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, int full_w,
     const uint32_t q = (blockIdx.x - (second ? blocks1 : 0u)) * blockDim.x + threadIdx.x;
     if (q >= (uint32_t)lv.cw * (uint32_t)lv.ch) return;
     const int Y = q / lv.cw, X = q - Y * lv.cw;
-    const int level = cell_level[(size_t)((Y * r) >> 3) * ((full_w + 7) >> 3) + ((X * r) >> 3)] & 3;
-    const uint8_t l2l[4] = {level_to_lod.x, level_to_lod.y, level_to_lod.z, level_to_lod.w};
-    if (l2l[level] != lod) return;
+    if (cell_level) {                                     // NULL: frame-global lod, every pixel
+        const int level = cell_level[(size_t)((Y * r) >> 3) * ((full_w + 7) >> 3) + ((X * r) >> 3)] & 3;
+        const uint8_t l2l[4] = {level_to_lod.x, level_to_lod.y, level_to_lod.z, level_to_lod.w};
+        if (l2l[level] != lod) return;
+    }
     const ColorT* __restrict__ rgba = static_cast<const ColorT*>(lv.rgba);
     const uint32_t b = __ldg(lv.offsets + q), e = __ldg(lv.offsets + q + 1);
     PixelState<false> s;
@@ -59,6 +61,23 @@ static noit_status check_desc(noit_ctx* ctx, const noit_resolve_desc* d, const c
         return noit_fail(ctx, NOIT_ERR_NULL, "%s: pixel_list and pixel_count go together", who);
     if (d->pixel_list && d->cell_level)
         return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "%s: pixel_list with cell_level", who);
+    if (d->pass_scales) {                                  // frame-global lod (O7g)
+        if (d->cell_level || d->pixel_list)
+            return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "%s: pass_scales with cell_level / pixel_list", who);
+        if (!noit_aligned(d->pass_scales, 4))
+            return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: pass_scales needs 4-byte alignment", who);
+        for (int lod = 1; lod <= 2; ++lod) {
+            const noit_fragbuf* cb = lod == 1 ? d->half : d->quarter;
+            if (!cb) return noit_fail(ctx, NOIT_ERR_NULL, "%s: pass_scales needs half and quarter", who);
+            NOIT_TRY(noit_check_fragbuf(ctx, cb, who));
+            const int r = 1 << lod;
+            if (cb->width != (d->full.width + r - 1) / r || cb->height != (d->full.height + r - 1) / r)
+                return noit_fail(ctx, NOIT_ERR_SIZE, "%s: lod %d buffer is not ceil(W/%d) x ceil(H/%d)",
+                                 who, lod, r, r);
+            if (cb->color_fmt != d->full.color_fmt)
+                return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: coarse buffers must share color_fmt", who);
+        }
+    }
     if (d->cell_level) {
         for (int l = 0; l < 4; ++l) {
             const int lod = d->level_to_lod[l];
@@ -100,7 +119,8 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
 
     if (d->pixel_list)                                     // S9: staged kernel, list mode
         return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_LIST, st);
-    if (d->cell_level) {                                   // S7
+    if (d->cell_level || d->pass_scales) {                 // S7 / frame-global lod
+        A.pass_scales = d->pass_scales;
         memcpy(A.level_to_lod, d->level_to_lod, 4);
         const uchar4 l2l = make_uchar4(d->level_to_lod[0], d->level_to_lod[1], d->level_to_lod[2],
                                        d->level_to_lod[3]);
@@ -108,7 +128,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
         memset(lv, 0, sizeof lv);
         uint32_t blocks[2] = {0, 0};
         for (int lod = 1; lod <= 2; ++lod) {
-            bool used = false;
+            bool used = d->pass_scales != nullptr;         // global: the lods are decided on the device
             for (int l = 0; l < 4; ++l) used |= d->level_to_lod[l] == lod;
             if (!used) continue;
             const noit_fragbuf* cb = lod == 1 ? d->half : d->quarter;

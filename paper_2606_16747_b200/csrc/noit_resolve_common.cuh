@@ -16,7 +16,8 @@ struct ResolveArgs {
     // S9
     const uint32_t* pixel_list;
     const uint32_t* pixel_count;
-    // S7
+    // S7 / frame-global LOD (O7g)
+    const float* pass_scales;      // device {w, s_2, s_3}: frame-global pass-2 / pass-3 lod
     const uint8_t* cell_level;
     uint8_t level_to_lod[4];
     const float* coarse_g[2];      // G[10] per coarse pixel, lod 1 (half) and lod 2 (quarter)

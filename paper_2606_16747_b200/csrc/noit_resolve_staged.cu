@@ -369,9 +369,17 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         }
     };
     // S7 (kMode ADAPTIVE): lod of the lane's pixel; a tile with any lod > 0 takes the mixed path
+    // frame-global lods of pass 2 / pass 3 from the Eq. 2 scales (O7g, A27), decided here
+    int g_lod2 = 0, g_lod3 = 0;
+    if (kMode == NOIT_RESOLVE_ADAPTIVE && A.pass_scales) {
+        const float s2 = __ldg(A.pass_scales + 1), s3 = __ldg(A.pass_scales + 2);
+        g_lod2 = s2 > 0.70710678f ? 0 : (s2 > 0.35355339f ? 1 : 2);
+        g_lod3 = s3 > 0.70710678f ? 0 : (s3 > 0.35355339f ? 1 : 2);
+    }
     auto lane_lod = [&](uint32_t pix, int& level) -> int {
         level = 3;
         if (kMode != NOIT_RESOLVE_ADAPTIVE || pix >= A.P) return 0;
+        if (A.pass_scales) return max(g_lod2, g_lod3);
         const uint32_t y = pix / (uint32_t)A.W, x = pix - y * (uint32_t)A.W;
         level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)] & 3;
         return A.level_to_lod[level];
@@ -493,7 +501,44 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             // accumulators bilinearly sampled from the coarse buffer's G (O7).
             const ColorT* rgba_t = static_cast<const ColorT*>(A.rgba);
             epi_ready = true;
-            if (lod == 0) {
+            if (A.pass_scales) {
+                // frame-global lods: layer 1 from the full list; pass 2 / pass 3 each from the
+                // pixel's own list (lod 0) or the coarse G of its lod, taps clamped to the image
+                const int y = (int)(pix / (uint32_t)A.W), x = (int)(pix - (uint32_t)y * (uint32_t)A.W);
+                float G2[10], G3[10];
+                PixelState<false> ps;
+                ps.init();
+                if (g_lod2 == 0 || g_lod3 == 0) {
+                    for (uint32_t j = o0; j < o1; ++j) ps.push(__ldg(A.depth + j), load_rgba(rgba_t, j), j);
+                    e_c1 = ps.c1;
+                    e_d1 = o1 > o0 ? ps.d1 : 1.0f;
+                } else {
+                    float d1 = __int_as_float(0x7f800000);
+                    uint32_t i1 = o0;
+                    for (uint32_t j = o0; j < o1; ++j) {
+                        const float d = __ldg(A.depth + j);
+                        if (d < d1) { d1 = d; i1 = j; }
+                    }
+                    if (o1 > o0) { e_c1 = load_rgba(rgba_t, i1); e_d1 = d1; }
+                }
+                if (g_lod2 > 0)
+                    sample_coarse_g(A.coarse_g[g_lod2 - 1], A.coarse_w[g_lod2 - 1], A.coarse_h[g_lod2 - 1],
+                                    1 << g_lod2, 1 << 30, x, y, G2);
+                if (g_lod3 > 0 && g_lod3 != g_lod2)
+                    sample_coarse_g(A.coarse_g[g_lod3 - 1], A.coarse_w[g_lod3 - 1], A.coarse_h[g_lod3 - 1],
+                                    1 << g_lod3, 1 << 30, x, y, G3);
+                e_l2 = g_lod2 == 0 ? make_float4(ps.c2.w * ps.c2.x, ps.c2.w * ps.c2.y, ps.c2.w * ps.c2.z, ps.c2.w)
+                                   : make_float4(G2[0], G2[1], G2[2], G2[3]);
+                if (g_lod3 == 0) {
+                    has_tail = make_features((float)(o1 - o0), ps.t_tail, ps.acc_r, ps.acc_g, ps.acc_b,
+                                             ps.a_tail, xf);
+                    e_tt = ps.t_tail;
+                } else {
+                    const float* T = g_lod3 == g_lod2 ? G2 : G3;
+                    has_tail = make_features(T[9], T[8], T[4], T[5], T[6], T[7], xf);
+                    e_tt = T[8];
+                }
+            } else if (lod == 0) {
                 PixelState<false> ps;
                 ps.init();
                 for (uint32_t j = o0; j < o1; ++j) ps.push(__ldg(A.depth + j), load_rgba(rgba_t, j), j);

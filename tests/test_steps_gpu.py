@@ -358,6 +358,49 @@ def test_quadtree_then_balance_on_cfg4(noit, cfg4_small):
     assert np.max(np.abs(got["scales"].cpu().numpy() - ref["scales"])) <= 1e-6
 
 
+@pytest.mark.parametrize("s2,s3", [(1.0, 1.0), (0.5, 0.5), (0.5, 0.25), (0.25, 0.25), (1.0, 0.25),
+                                   (1.0, 0.5), (0.25, 0.5), (0.8, 0.36)])
+def test_frame_global_pass_resolution(noit, cfg4_small, s2, s3):
+    """O7g: pass 2 / pass 3 lods for the whole frame, snapped on the device from the scales."""
+    sc = cfg4_small
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    scales = torch.tensor([2.0, s2, s3], dtype=torch.float32, device="cuda")
+    got = ctx.resolve(fb, BG, half=hb, quarter=qb, pass_scales=scales)
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    ref = oracle.resolve_global(sc.full, sc.half, sc.quarter, w_eff, BG, oracle.snap_lod(s2),
+                                oracle.snap_lod(s3))
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    lay = oracle.build_features(sc.full)
+    mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=extra)
+        assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
+
+
+def test_frame_global_chain_from_device_scales(noit, cfg4_small):
+    """quadtree -> balance (w, s_2, s_3 on the device) -> resolve at those pass resolutions, with
+    no host round trip between the calls."""
+    sc = cfg4_small
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    img = ctx.resolve(fb, BG)["final"]
+    qt = ctx.quadtree(img, fb.width, fb.height, var_threshold_q=6)
+    bal = ctx.quadtree_balance(qt["tile_mask"], fb.width, fb.height)
+    got = ctx.resolve(fb, BG, half=hb, quarter=qb, pass_scales=bal["scales"])
+    sc_host = bal["scales"].cpu().numpy()
+    lod2, lod3 = oracle.snap_lod(sc_host[1]), oracle.snap_lod(sc_host[2])
+    assert lod3 >= lod2                                                        # delta_3 > delta_2
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    ref = oracle.resolve_global(sc.full, sc.half, sc.quarter, w_eff, BG, lod2, lod3)
+    lay = oracle.build_features(sc.full)
+    mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=extra)
+
+
 # -------------------------------------------------------------------------------------------
 # NEXT-2: temporal tile state (O11)
 # -------------------------------------------------------------------------------------------
