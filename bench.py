@@ -367,6 +367,72 @@ def cpu_baseline(sc) -> dict:
             "sample": f"plain resolve (S1-S5) of the whole cfg3 frame, {n} repetitions"}
 
 
+def run_info(args):
+    """`--config cfgK` (information only, not the contract line): the plain resolve -- and for cfg4
+    the quadtree + balance + adaptive resolve -- of BASELINE.json's other configs, CUDA-event means
+    with an L2 flush (a 512 MB fill) between iterations where the inputs fit L2."""
+    import torch
+
+    import noit_scenes
+    import paper_2606_16747_b200 as noit
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    name = args.config
+    if name == "cfg5":
+        seq = noit_scenes.cfg5(0)
+        sc = noit_scenes.Scene("cfg5-frame0", seq.frame(0), weights=seq.weights, mlp_precision=seq.mlp_precision)
+    else:
+        sc = {"cfg1": noit_scenes.cfg1, "cfg2": noit_scenes.cfg2, "cfg3": noit_scenes.cfg3,
+              "cfg4": noit_scenes.cfg4}[name](0)
+    fbh = sc.full
+    P, F = fbh.num_pixels, fbh.num_fragments
+    cb = fbh.rgba.dtype.itemsize * 4
+    fb = noit.DeviceFragBuf.from_host(fbh, dev)
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    f32 = dict(dtype=torch.float32, device=dev)
+    out = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
+    d_plain = ctx.make_resolve_desc(fb, BG, out["trans"], out["final"], out["depth1"])
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, n):
+        for _ in range(3):
+            fn()
+        ms = []
+        for _ in range(n):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            ms.append(a.elapsed_time(b))
+        return float(np.mean(ms))
+
+    peak, peak_src = peaks()
+    rec = {"info": True, "config": name, "pixels": P, "fragments": F, "steps": args.steps,
+           "l2": "512 MB fill between iterations"}
+    t = timed(lambda: ctx.resolve_desc(d_plain), args.steps)
+    rbytes = resolve_bytes(P, F, cb, 2, True)
+    rec.update(resolve_ms=t, resolve_mpix_s=P / t / 1e3, resolve_gfrag_s=F / t / 1e6,
+               resolve_gbs=rbytes / t / 1e6, resolve_frac_of_hbm_peak=rbytes / t / 1e6 / peak,
+               mlp_us_at_fp32_peak=P * 1440 / 74.4e12 * 1e6, peak_source=peak_src)
+    if sc.half is not None:
+        hb, qb = (noit.DeviceFragBuf.from_host(b, dev) for b in (sc.half, sc.quarter))
+        W, H = fbh.width, fbh.height
+        qt = ctx.quadtree(out["final"], W, H, noit.QT_VARIANCE, 6)
+        bal = ctx.quadtree_balance(qt["tile_mask"], W, H)
+        adapt = dict(final=torch.empty((P, 4), **f32))
+        ta = timed(lambda: ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb,
+                                       cell_level=bal["cell_level"]), args.steps)
+        lv = bal["cell_level"].cpu().numpy()
+        rec.update(adaptive_ms=ta, adaptive_speedup_over_plain=t / ta,
+                   tile_hist=bal["hist"].cpu().numpy().view(np.uint32).tolist(),
+                   cell_fraction_per_level=[float((lv == k).mean()) for k in range(4)],
+                   scales=[float(v) for v in bal["scales"].cpu().numpy()])
+    print(json.dumps(rec))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -374,11 +440,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--config", default=None, choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"],
+                    help="information only: time one of BASELINE.json's other configs")
     args = ap.parse_args()
     if os.environ.get("NOIT_BENCH_DRYRUN"):
         return run_dryrun(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.config:
+        return run_info(args)
     return run_ours(args)
 
 

@@ -6,7 +6,7 @@
 noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt, int mode,
                                        cudaStream_t st);
 
-// S7 pre-pass: G[10] of every coarse pixel whose leaf is resolved at that lod (self-contained
+// S7 pre-pass: G (10 values in 12 floats) of every coarse pixel whose leaf is resolved at that lod (self-contained
 // O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
 // One launch covers both coarse levels: blocks [0, blocks1) the half-res buffer (lod 1), the rest
 // the quarter-res buffer (lod 2).
@@ -38,10 +38,10 @@ coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, int full_w,
     PixelState<false> s;
     s.init();
     for (uint32_t j = b; j < e; ++j) s.push(__ldg(lv.depth + j), load_rgba(rgba, j), j);
-    float* g = lv.G + 10 * (size_t)q;
-    g[0] = s.c2.w * s.c2.x; g[1] = s.c2.w * s.c2.y; g[2] = s.c2.w * s.c2.z; g[3] = s.c2.w;
-    g[4] = s.acc_r; g[5] = s.acc_g; g[6] = s.acc_b; g[7] = s.a_tail; g[8] = s.t_tail;
-    g[9] = (float)(e - b);
+    float4* g = reinterpret_cast<float4*>(lv.G) + 3 * (size_t)q;
+    g[0] = make_float4(s.c2.w * s.c2.x, s.c2.w * s.c2.y, s.c2.w * s.c2.z, s.c2.w);
+    g[1] = make_float4(s.acc_r, s.acc_g, s.acc_b, s.a_tail);
+    g[2] = make_float4(s.t_tail, (float)(e - b), 0.f, 0.f);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -140,7 +140,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
                     ctx->d_coarse_g[lod - 1] = nullptr;
                     ctx->coarse_g_cap[lod - 1] = 0;
                 }
-                NOIT_CUDA(ctx, cudaMalloc(&ctx->d_coarse_g[lod - 1], cp * 10 * sizeof(float)));
+                NOIT_CUDA(ctx, cudaMalloc(&ctx->d_coarse_g[lod - 1], cp * NOIT_G_STRIDE * sizeof(float)));
                 ctx->coarse_g_cap[lod - 1] = cp;
             }
             A.coarse_g[lod - 1] = ctx->d_coarse_g[lod - 1];

@@ -34,32 +34,42 @@ enum { NOIT_RESOLVE_ALL = 0, NOIT_RESOLVE_LIST = 1, NOIT_RESOLVE_ADAPTIVE = 2 };
 // lod > 0 pixel of S7 (O7): bilinear sample of G = [a2*C2 (3), a2, C_acc (3), A_tail, T_tail, N]
 // at the full-res pixel centre, taps clamped to the coarse texels of the pixel's own leaf and to
 // the image (A19).  lerp(a,b,w) = a + w(b-a), x first then y; the weights are dyadic.
-__device__ __forceinline__ void sample_coarse_g(const float* __restrict__ G, int cw, int ch, int r,
-                                                int leaf_side, int x, int y, float out[10])
+// G is stored as 12 floats (three float4) per coarse pixel: [a2*C2 (3), a2, C_acc (3), A_tail,
+// T_tail, N, pad, pad].  r = 1 << lod; the leaf side is 1 << leaf_shift pixels (both powers of two:
+// shifts, no integer divisions).
+#define NOIT_G_STRIDE 12
+__device__ __forceinline__ void sample_coarse_g(const float* __restrict__ G, int cw, int ch, int lod,
+                                                int leaf_shift, int x, int y, float out[10])
 {
-    const float inv_r = 1.f / (float)r;
+    const float inv_r = lod == 1 ? 0.5f : 0.25f;
     const float u = ((float)x + 0.5f) * inv_r - 0.5f, v = ((float)y + 0.5f) * inv_r - 0.5f;
     const float fu = floorf(u), fv = floorf(v);
     const int i0 = (int)fu, j0 = (int)fv;
     const float wx = u - fu, wy = v - fv;
-    const int lx0 = (x / leaf_side) * leaf_side, ly0 = (y / leaf_side) * leaf_side;
-    const int tx_lo = lx0 / r, ty_lo = ly0 / r;
-    const int tx_hi = min((lx0 + leaf_side - 1) / r, cw - 1);
-    const int ty_hi = min((ly0 + leaf_side - 1) / r, ch - 1);
+    const int lx0 = (x >> leaf_shift) << leaf_shift, ly0 = (y >> leaf_shift) << leaf_shift;
+    const int leaf_last = (1 << leaf_shift) - 1;
+    const int tx_lo = lx0 >> lod, ty_lo = ly0 >> lod;
+    const int tx_hi = min((lx0 + leaf_last) >> lod, cw - 1);
+    const int ty_hi = min((ly0 + leaf_last) >> lod, ch - 1);
     const int xa = min(max(i0, tx_lo), tx_hi), xb = min(max(i0 + 1, tx_lo), tx_hi);
     const int ya = min(max(j0, ty_lo), ty_hi), yb = min(max(j0 + 1, ty_lo), ty_hi);
-    const float* g00 = G + 10 * ((size_t)ya * cw + xa);
-    const float* g10 = G + 10 * ((size_t)ya * cw + xb);
-    const float* g01 = G + 10 * ((size_t)yb * cw + xa);
-    const float* g11 = G + 10 * ((size_t)yb * cw + xb);
+    const float4* g00 = reinterpret_cast<const float4*>(G) + 3 * ((size_t)ya * cw + xa);
+    const float4* g10 = reinterpret_cast<const float4*>(G) + 3 * ((size_t)ya * cw + xb);
+    const float4* g01 = reinterpret_cast<const float4*>(G) + 3 * ((size_t)yb * cw + xa);
+    const float4* g11 = reinterpret_cast<const float4*>(G) + 3 * ((size_t)yb * cw + xb);
 #pragma unroll
-    for (int k = 0; k < 10; ++k) {
-        const float a = g00[k], b = g10[k], c = g01[k], d = g11[k];
-        const float top = fmaf(wx, b - a, a), bot = fmaf(wx, d - c, c);
-        out[k] = fmaf(wy, bot - top, top);
+    for (int q = 0; q < 3; ++q) {
+        const float4 A4 = __ldg(g00 + q), B4 = __ldg(g10 + q), C4 = __ldg(g01 + q), D4 = __ldg(g11 + q);
+        const float a[4] = {A4.x, A4.y, A4.z, A4.w}, b[4] = {B4.x, B4.y, B4.z, B4.w};
+        const float c[4] = {C4.x, C4.y, C4.z, C4.w}, d[4] = {D4.x, D4.y, D4.z, D4.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (4 * q + k >= 10) continue;
+            const float top = fmaf(wx, b[k] - a[k], a[k]), bot = fmaf(wx, d[k] - c[k], c[k]);
+            out[4 * q + k] = fmaf(wy, bot - top, top);
+        }
     }
 }
-
 // O5 / Eq. 4.  c1 = straight RGBA of layer 1; l2 = PREMULTIPLIED layer 2
 // (a2*C2, a2); absent layers are all-zero (A10).  f is ignored when has_tail is false (A2).
 __device__ __forceinline__ void composite_store(const ResolveArgs& A, uint32_t p, float4 c1,

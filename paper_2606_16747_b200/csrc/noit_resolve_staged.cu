@@ -368,7 +368,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             b = __ldg(offsets + min(pix + 1u, A.P));
         }
     };
-    // S7 (kMode ADAPTIVE): lod of the lane's pixel; a tile with any lod > 0 takes the mixed path
+    // S7 (kMode ADAPTIVE): lod of a pixel.  Every tile runs the staged path; pixels with lod > 0
+    // then take layer 2 / the tail from the coarse G in the epilogue, and a tile whose pixels ALL
+    // do stages only its depths.
     // frame-global lods of pass 2 / pass 3 from the Eq. 2 scales (O7g, A27), decided here
     int g_lod2 = 0, g_lod3 = 0;
     if (kMode == NOIT_RESOLVE_ADAPTIVE && A.pass_scales) {
@@ -433,12 +435,14 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         for (int r = 0; r < L; ++r) fits = fits && (B[r + 1] - (B[r] & ~3u) <= kCapC);
         return fits;
     };
-    auto first_fill = [&](uint32_t a, uint32_t b, bool unstaged) {
-        if (kMode == NOIT_RESOLVE_LIST || unstaged) return;
+    auto first_fill = [&](uint32_t a, uint32_t b, bool depth_only_tile) {
+        if (kMode == NOIT_RESOLVE_LIST) return;
         const uint32_t tb = __shfl_sync(0xffffffffu, a, 0), te = __shfl_sync(0xffffffffu, b, 31);
         const uint32_t fs = tb & ~3u;
         if (te <= tb) return;
-        if (te - fs <= kCap) {
+        if (depth_only_tile && te - fs <= kCapD) {
+            issue_fill(sD, nullptr, fs, te);
+        } else if (te - fs <= kCap) {
             issue_fill(sD, sC2, fs, te);
         } else {
             uint32_t B[L + 1], bk;
@@ -454,13 +458,19 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     uint32_t raw_nxt = warp_id + n_warps, raw_nn = warp_id + 2u * n_warps;   // then two atomics in flight
     uint32_t o0 = 0, o1 = 0, pix = 0;
     int lod = 0, level = 3;
-    bool mixed = false;                                  // S7: the tile has pixels with lod > 0
+    bool mixed = false;                                  // S7 / O7g: some pixel of the tile has lod > 0
+    bool depth_only = false;                             // ... every pixel takes layer 2 AND tail coarse
+    // a lane whose pixel needs nothing but layer 1 from the full-resolution list
+    auto coarse_lane = [&](uint32_t pixel, int l) -> bool {
+        return pixel >= A.P || (A.pass_scales ? (g_lod2 > 0 && g_lod3 > 0) : l > 0);
+    };
     if (t_cur < num_tiles) {
         pix = lane_pixel(t_cur);
         load_offsets(pix, o0, o1);
         lod = lane_lod(pix, level);
         mixed = __any_sync(0xffffffffu, lod > 0);
-        first_fill(o0, o1, mixed);
+        depth_only = mixed && __all_sync(0xffffffffu, coarse_lane(pix, lod));
+        first_fill(o0, o1, depth_only);
     }
     while (t_cur < num_tiles) {
         const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
@@ -480,11 +490,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
         uint32_t px_own = lane;                          // pixel of the tile this lane ends up owning
 
-        // inputs of the epilogue when a path produces them directly (S7 mixed tiles)
+        // inputs of the epilogue
         float xf[5];
         float4 e_c1 = make_float4(0.f, 0.f, 0.f, 0.f), e_l2 = e_c1;
         float e_d1 = 1.0f, e_tt = 1.0f;
-        bool has_tail = false, epi_ready = false;
+        bool has_tail = false;
 
         const uint32_t tb = __shfl_sync(0xffffffffu, o0, 0), te = __shfl_sync(0xffffffffu, o1, 31);
         const uint32_t fs = tb & ~3u;
@@ -494,75 +504,16 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             // every warp of the machine busy); lanes with lane % L == 0 own a pixel
             px_own = (uint32_t)(lane / L);
             own = tile_from_global<ColorT, L, 1>(lane, o0, o1, A.depth, g_rgba);
-        } else if (kMode == NOIT_RESOLVE_ADAPTIVE && mixed) {
-            // ---- S7 tile with coarse pixels (smooth regions: few fragments): one lane per pixel
-            // straight from global memory.  lod 0 lanes: O1-O3; lod > 0 lanes: layer 1 from the
-            // full buffer (depth-only scan + one colour fetch), layer 2 and the raw tail
-            // accumulators bilinearly sampled from the coarse buffer's G (O7).
-            const ColorT* rgba_t = static_cast<const ColorT*>(A.rgba);
-            epi_ready = true;
-            if (A.pass_scales) {
-                // frame-global lods: layer 1 from the full list; pass 2 / pass 3 each from the
-                // pixel's own list (lod 0) or the coarse G of its lod, taps clamped to the image
-                const int y = (int)(pix / (uint32_t)A.W), x = (int)(pix - (uint32_t)y * (uint32_t)A.W);
-                float G2[10], G3[10];
-                PixelState<false> ps;
-                ps.init();
-                if (g_lod2 == 0 || g_lod3 == 0) {
-                    for (uint32_t j = o0; j < o1; ++j) ps.push(__ldg(A.depth + j), load_rgba(rgba_t, j), j);
-                    e_c1 = ps.c1;
-                    e_d1 = o1 > o0 ? ps.d1 : 1.0f;
-                } else {
-                    float d1 = __int_as_float(0x7f800000);
-                    uint32_t i1 = o0;
-                    for (uint32_t j = o0; j < o1; ++j) {
-                        const float d = __ldg(A.depth + j);
-                        if (d < d1) { d1 = d; i1 = j; }
-                    }
-                    if (o1 > o0) { e_c1 = load_rgba(rgba_t, i1); e_d1 = d1; }
-                }
-                if (g_lod2 > 0)
-                    sample_coarse_g(A.coarse_g[g_lod2 - 1], A.coarse_w[g_lod2 - 1], A.coarse_h[g_lod2 - 1],
-                                    1 << g_lod2, 1 << 30, x, y, G2);
-                if (g_lod3 > 0 && g_lod3 != g_lod2)
-                    sample_coarse_g(A.coarse_g[g_lod3 - 1], A.coarse_w[g_lod3 - 1], A.coarse_h[g_lod3 - 1],
-                                    1 << g_lod3, 1 << 30, x, y, G3);
-                e_l2 = g_lod2 == 0 ? make_float4(ps.c2.w * ps.c2.x, ps.c2.w * ps.c2.y, ps.c2.w * ps.c2.z, ps.c2.w)
-                                   : make_float4(G2[0], G2[1], G2[2], G2[3]);
-                if (g_lod3 == 0) {
-                    has_tail = make_features((float)(o1 - o0), ps.t_tail, ps.acc_r, ps.acc_g, ps.acc_b,
-                                             ps.a_tail, xf);
-                    e_tt = ps.t_tail;
-                } else {
-                    const float* T = g_lod3 == g_lod2 ? G2 : G3;
-                    has_tail = make_features(T[9], T[8], T[4], T[5], T[6], T[7], xf);
-                    e_tt = T[8];
-                }
-            } else if (lod == 0) {
-                PixelState<false> ps;
-                ps.init();
-                for (uint32_t j = o0; j < o1; ++j) ps.push(__ldg(A.depth + j), load_rgba(rgba_t, j), j);
-                has_tail = make_features((float)(o1 - o0), ps.t_tail, ps.acc_r, ps.acc_g, ps.acc_b,
-                                         ps.a_tail, xf);
-                e_c1 = ps.c1;
-                e_l2 = make_float4(ps.c2.w * ps.c2.x, ps.c2.w * ps.c2.y, ps.c2.w * ps.c2.z, ps.c2.w);
-                e_d1 = o1 > o0 ? ps.d1 : 1.0f;
-                e_tt = ps.t_tail;
-            } else {
-                float d1 = __int_as_float(0x7f800000);
-                uint32_t i1 = o0;
-                for (uint32_t j = o0; j < o1; ++j) {
-                    const float d = __ldg(A.depth + j);
-                    if (d < d1) { d1 = d; i1 = j; }
-                }
-                if (o1 > o0) { e_c1 = load_rgba(rgba_t, i1); e_d1 = d1; }
-                const int y = (int)(pix / (uint32_t)A.W), x = (int)(pix - (uint32_t)y * (uint32_t)A.W);
-                float G[10];
-                sample_coarse_g(A.coarse_g[lod - 1], A.coarse_w[lod - 1], A.coarse_h[lod - 1], 1 << lod,
-                                64 >> level, x, y, G);
-                has_tail = make_features(G[9], G[8], G[4], G[5], G[6], G[7], xf);
-                e_l2 = make_float4(G[0], G[1], G[2], G[3]);
-                e_tt = G[8];
+        } else if (kMode == NOIT_RESOLVE_ADAPTIVE && depth_only && te - fs <= kCapD) {
+            // ---- S7 / O7g tile whose 32 pixels all take layer 2 and the tail from a coarse buffer:
+            // only layer 1 is needed from the full-resolution lists, so only the DEPTHS are
+            // staged (4 of the 12 bytes per fragment) and the winner's colour is fetched directly
+            if (te > tb) {
+                wait_fill();
+                const Top2 s = scan_depths<1>(sD, o0 - fs, o1 - fs);
+                if (s.i1 != NOIT_ABSENT) own.c1 = __ldg(g_rgba + fs + s.i1);
+                own.d1 = s.d1;
+                own.n = o1 - o0;
             }
         } else if (te - fs <= kCap) {
             // ---- light tile: one lane per pixel, depths and colours staged together
@@ -657,13 +608,14 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         }
         // (the vote is taken here, not where the level was requested: it would wait for the load)
         const bool nmixed = kMode == NOIT_RESOLVE_ADAPTIVE && __any_sync(0xffffffffu, nlod > 0);
-        if (t_nxt < num_tiles) first_fill(no0, no1, nmixed);
+        const bool ndepth_only = nmixed && __all_sync(0xffffffffu, coarse_lane(npix, nlod));
+        if (t_nxt < num_tiles) first_fill(no0, no1, ndepth_only);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
         uint32_t p = __shfl_sync(0xffffffffu, pix, (int)px_own);
         if (kMode == NOIT_RESOLVE_LIST && (lane % L) != 0) p = 0xFFFFFFFFu;   // not an owner
         {
             float f[3];
-            if (!epi_ready) {
+            {
                 // O3 with one IEEE reciprocal instead of three divisions
                 has_tail = own.a_tail > 0.f;
                 const float inv = has_tail ? 1.0f / own.a_tail : 0.f;
@@ -675,11 +627,40 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 e_d1 = own.n ? own.d1 : 1.0f;
                 e_tt = own.t_tail;
             }
+            if (kMode == NOIT_RESOLVE_ADAPTIVE && mixed && p < A.P) {
+                // S7 / O7g: layer 2 and / or the raw tail accumulators of this pixel come from a
+                // coarse buffer's G, bilinearly sampled at the pixel centre; layer 1 stays
+                // the full-resolution one
+                int plevel;
+                const int plod = lane_lod(p, plevel);                // of the OWNED pixel
+                const int y = (int)(p / (uint32_t)A.W), x = (int)(p - (uint32_t)y * (uint32_t)A.W);
+                float G2[10], G3[10];
+                if (A.pass_scales) {                                 // frame-global lods, image clamp
+                    if (g_lod2 > 0)
+                        sample_coarse_g(A.coarse_g[g_lod2 - 1], A.coarse_w[g_lod2 - 1], A.coarse_h[g_lod2 - 1],
+                                        g_lod2, 30, x, y, G2);
+                    if (g_lod3 > 0 && g_lod3 != g_lod2)
+                        sample_coarse_g(A.coarse_g[g_lod3 - 1], A.coarse_w[g_lod3 - 1], A.coarse_h[g_lod3 - 1],
+                                        g_lod3, 30, x, y, G3);
+                    if (g_lod2 > 0) e_l2 = make_float4(G2[0], G2[1], G2[2], G2[3]);
+                    if (g_lod3 > 0) {
+                        const float* T = g_lod3 == g_lod2 ? G2 : G3;
+                        has_tail = make_features(T[9], T[8], T[4], T[5], T[6], T[7], xf);
+                        e_tt = T[8];
+                    }
+                } else if (plod > 0) {                               // per-tile lod, leaf clamp
+                    sample_coarse_g(A.coarse_g[plod - 1], A.coarse_w[plod - 1], A.coarse_h[plod - 1],
+                                    plod, 6 - plevel, x, y, G2);
+                    e_l2 = make_float4(G2[0], G2[1], G2[2], G2[3]);
+                    has_tail = make_features(G2[9], G2[8], G2[4], G2[5], G2[6], G2[7], xf);
+                    e_tt = G2[8];
+                }
+            }
             if (kMma) mlp_forward_mma(wv, scratch, lane, xf, f);     // all 32 lanes
             else mlp_forward_packed(W, xf, f);
             if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
-        pix = npix; lod = nlod; level = nlevel; mixed = nmixed;
+        pix = npix; lod = nlod; level = nlevel; mixed = nmixed; depth_only = ndepth_only;
         t_cur = t_nxt; o0 = no0; o1 = no1;
     }
     // the last warp to finish re-arms the counters for the next launch
