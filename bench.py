@@ -425,6 +425,11 @@ def run_info(args):
         adapt = dict(final=torch.empty((P, 4), **f32))
         ta = timed(lambda: ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb,
                                        cell_level=bal["cell_level"]), args.steps)
+        # the paper's frame-global control with pass 2 at half and pass 3 at quarter resolution
+        forced = torch.tensor([2.0, 0.5, 0.25], **f32)
+        tg = timed(lambda: ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, pass_scales=forced),
+                   args.steps)
+        rec.update(global_half_quarter_ms=tg, global_speedup_over_plain=t / tg)
         lv = bal["cell_level"].cpu().numpy()
         rec.update(adaptive_ms=ta, adaptive_speedup_over_plain=t / ta,
                    tile_hist=bal["hist"].cpu().numpy().view(np.uint32).tolist(),
