@@ -67,6 +67,17 @@ def infer(weights_eff: np.ndarray, features: np.ndarray) -> np.ndarray:
     return out
 
 
+def infer10(weights931: np.ndarray, features: np.ndarray) -> np.ndarray:
+    """The 10-feature, sigmoid-output network DFAOIT uses (931 parameters; comparison variant)."""
+    f = np.ascontiguousarray(features, np.float32)
+    n = f.shape[0]
+    assert f.shape[1] == 10
+    out = np.empty((n, 3), np.float32)
+    rc = lib().oracle_infer10(_p(_chk(weights931, np.float32, 931)), _p(f), C.c_uint32(n), _p(out))
+    assert rc == 0
+    return out
+
+
 def _fb_args(fb):
     if fb is None:
         return [C.c_int32(0), C.c_int32(0), None, None, None]

@@ -175,6 +175,39 @@ int32_t oracle_infer(const float *weights, const float *features, uint32_t n, fl
     return 0;
 }
 
+/* NEXT-4 (comparison variant): the network DFAOIT feeds with 10 input features and  */
+/* a SIGMOID output, "the architecture differs only in the output activation":           */
+/* 10 -> 32 -> 16 -> 3 = 931 parameters, W1[32][10], b1[32], W2[16][32], b2[16], W3[3][16],     */
+/* b3[3].  Only the network is built (inference-cost ratio 10 -> 5 features); what the  */
+/* ten features ARE is only summarised in this paper: parity of the inputs unpinned.   */
+int32_t oracle_infer10(const float *w, const float *features, uint32_t n, float *rgb)
+{
+    if (!w || !features || !rgb) return 1;
+    const float *W1 = w, *b1 = W1 + 32 * 10, *W2 = b1 + 32, *b2 = W2 + 16 * 32;
+    const float *W3 = b2 + 16, *b3 = W3 + 3 * 16;
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < (int64_t)n; ++r) {
+        const float *x = features + 10 * r;
+        double h1[32], h2[16];
+        for (int o = 0; o < 32; ++o) {
+            double a = (double)b1[o];
+            for (int i = 0; i < 10; ++i) a += (double)W1[o * 10 + i] * (double)x[i];
+            h1[o] = a > 0.0 ? a : 0.0;
+        }
+        for (int o = 0; o < 16; ++o) {
+            double a = (double)b2[o];
+            for (int i = 0; i < 32; ++i) a += (double)W2[o * 32 + i] * h1[i];
+            h2[o] = a > 0.0 ? a : 0.0;
+        }
+        for (int o = 0; o < 3; ++o) {
+            double a = (double)b3[o];
+            for (int i = 0; i < 16; ++i) a += (double)W3[o * 16 + i] * h2[i];
+            rgb[3 * r + o] = (float)(1.0 / (1.0 + exp(-a)));
+        }
+    }
+    return 0;
+}
+
 /* ---------------------------------------------------------------------------------------- */
 /* S1-S3: layers, tail accumulators, features for every pixel                                */
 /* ---------------------------------------------------------------------------------------- */

@@ -913,3 +913,35 @@ def test_global_lod_upsamples_an_affine_layer2_alpha_exactly():
     want = (1 - a1) * (1 - (0.1 + 0.05 * u))
     got = out["trans"].reshape(H, W, 4)[..., 3]
     assert np.allclose(got, np.tile(want, (H, 1)), rtol=1e-6, atol=1e-7)
+
+
+# -------------------------------------------------------------------------------------------
+# NEXT-4: the 10-feature / sigmoid network of the comparison system
+# -------------------------------------------------------------------------------------------
+def _weights931(seed):
+    rng = np.random.default_rng(seed)
+    parts = []
+    for fan_in, fan_out in ((10, 32), (32, 16), (16, 3)):
+        bound = 1.0 / np.sqrt(fan_in)
+        parts += [rng.uniform(-bound, bound, (fan_out, fan_in)).ravel(), rng.uniform(-bound, bound, fan_out)]
+    return np.concatenate(parts).astype(np.float32)
+
+
+def test_infer10_vs_numpy_and_parameter_count():
+    w = _weights931(3)
+    assert w.size == 931                                   # the count the paper's 10-input net has
+    rng = np.random.default_rng(9)
+    x = rng.random((500, 10)).astype(np.float32)
+    x[:, 9] = rng.integers(0, 129, 500)
+    w64 = w.astype(np.float64)
+    W1, b1 = w64[:320].reshape(32, 10), w64[320:352]
+    W2, b2 = w64[352:864].reshape(16, 32), w64[864:880]
+    W3, b3 = w64[880:928].reshape(3, 16), w64[928:931]
+    h = np.maximum(x.astype(np.float64) @ W1.T + b1, 0)
+    h = np.maximum(h @ W2.T + b2, 0)
+    want = 1.0 / (1.0 + np.exp(-(h @ W3.T + b3)))
+    got = oracle.infer10(w, x)
+    assert close(got, want, 1e-6, 1e-7)
+    z = np.zeros(931, np.float32)
+    z[928:] = [0.0, 1.0, -2.0]                             # zero weights: sigmoid of the bias
+    assert close(oracle.infer10(z, x)[0], 1 / (1 + np.exp(-np.array([0.0, 1.0, -2.0]))), 1e-6, 1e-7)
