@@ -311,7 +311,18 @@ def run_ours(args):
         tq["o"] = ctx.quadtree_temporal(plain["final"], W, H, qt["tile_mask"], out=tq["o"])
     def run_q16():
         q16["o"] = ctx.quadtree16(plain["final"], W, H, noit.QT_CORNER, 6, 0.02, out=q16["o"])
-    extras = {"quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
+    # NEXT-4: inference cost of the 5-feature network vs the comparison system's 10-feature one
+    # (same kernel shape; the paper reports a 35 % inference speed-up on RTX 5080)
+    rng10 = np.random.default_rng(1)
+    w931 = rng10.uniform(-0.2, 0.2, 931).astype(np.float32)
+    x5 = torch.rand((P, 5), **f32)
+    x10 = torch.rand((P, 10), **f32)
+    y3 = torch.empty((P, 3), **f32)
+    t5 = timed(lambda: ctx.infer(x5, out=y3))
+    t10 = timed(lambda: ctx.infer_dfaoit(w931, x10, out=y3))
+    extras = {"infer_5_features": t5, "infer_10_features_dfaoit": t10,
+              "inference_time_saved_by_5_features": 1.0 - t5 / t10,
+              "quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
               "quadtree_balance": timed(lambda: ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal))}
     clocks = sampler.stop() if rank == 0 else None
     rejected = int(rp["reject_count"].item())

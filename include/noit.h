@@ -54,6 +54,7 @@ enum { NOIT_MLP_FP32 = 0, NOIT_MLP_BF16 = 1 };     /* weight precision (A6)     
 enum { NOIT_QT_VARIANCE = 0, NOIT_QT_CORNER = 1 }; /* quadtree split metric (A14)             */
 
 #define NOIT_MLP_PARAMS 771        /* 5->32->16->3 with biases (A4)                     */
+#define NOIT_DFAOIT_PARAMS 931     /* 10->32->16->3: the comparison system's network   */
 #define NOIT_ABSENT 0xFFFFFFFFu    /* idx1/idx2 of a missing layer                            */
 
 typedef struct {
@@ -103,6 +104,16 @@ noit_status noit_build_features(noit_ctx* ctx, const noit_fragbuf* fb, const noi
  * No has_tail gating.  features [n][5] -> tail_rgb [n][3].  n == 0 is a no-op.               */
 noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* tail_rgb,
                        void* stream);
+
+/* ---- NEXT-4 (comparison variant): the network the comparison system DFAOIT evaluates, 10 input
+ * features -> 32 -> 16 -> 3 with a SIGMOID output ("differs only in the output activation",
+ * P:99-104), 931 parameters laid out W1[32][10], b1[32], W2[16][32], b2[16], W3[3][16], b3[3]
+ * in HOST memory (fp32, used as given).  It exists to measure the inference-cost ratio of the
+ * 10 -> 5 feature reduction with the same kernel shape as noit_infer; how DFAOIT forms
+ * its ten features is only summarised in the paper, so nothing here computes them.
+ * features [n][10] -> rgb [n][3] (device).  n == 0 is a no-op.                               */
+noit_status noit_infer_dfaoit(noit_ctx* ctx, const float* host_w, int32_t count, const float* features,
+                              uint32_t n, float* rgb, void* stream);
 
 /* ---- S1-S5 fused resolve (Eq. 4; O5); S7 when cell_level is set (O7);
  * S9 when pixel_list is set (O9).

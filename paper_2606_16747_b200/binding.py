@@ -22,7 +22,7 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
-           "noit_quadtree_balance", "noit_quadtree16",
+           "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit",
            "noit_reproject"]
 
 
@@ -198,6 +198,19 @@ class Noit:
             out = torch.empty((n, 3), dtype=torch.float32, device=features.device)
         self._check(self._L.noit_infer(self._ctx, _ptr(features), C.c_uint32(n), _ptr(out),
                                        _stream(stream)))
+        return out
+
+    # ---- NEXT-4 (comparison variant) ------------------------------------------------------
+    def infer_dfaoit(self, weights931, features: torch.Tensor, out=None, stream=None) -> torch.Tensor:
+        """10-feature / sigmoid-output network (931 host parameters) on [n, 10] device features."""
+        import numpy as np
+        w = np.ascontiguousarray(weights931, np.float32)
+        assert features.dtype == torch.float32 and features.is_contiguous()
+        n = features.shape[0]
+        if out is None:
+            out = torch.empty((n, 3), dtype=torch.float32, device=features.device)
+        self._check(self._L.noit_infer_dfaoit(self._ctx, w.ctypes.data_as(C.c_void_p), C.c_int32(w.size),
+                                              _ptr(features), C.c_uint32(n), _ptr(out), _stream(stream)))
         return out
 
     # ---- S1-S5 (+S7, +S9) ---------------------------------------------------------------

@@ -50,7 +50,69 @@ infer_kernel(const __grid_constant__ MlpWeights W, const float* __restrict__ fea
     for (int k = 0; k < 3; ++k) tail_rgb[3 * (size_t)r + k] = f[k];
 }
 
+// NEXT-4: the comparison system's network, 10 -> 32 -> 16 -> 3 with a sigmoid output (
+// 931 parameters).  Same shape of kernel as infer_kernel: one row per thread, weights as
+// constant-bank operands of the FFMAs, dot products from the bias in input-index order.
+struct MlpWeights10 {
+    float w1[32][10];
+    float b1[32];
+    float w2[16][32];
+    float b2[16];
+    float w3[3][16];
+    float b3[3];
+};
+static_assert(sizeof(MlpWeights10) == NOIT_DFAOIT_PARAMS * 4, "931 parameters");
+
+__global__ void __launch_bounds__(128)
+infer10_kernel(const __grid_constant__ MlpWeights10 W, const float* __restrict__ features, uint32_t n,
+               float* __restrict__ rgb)
+{
+    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    float x[10], h1[32], h2[16];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) x[k] = __ldg(features + 10 * (size_t)r + k);
+#pragma unroll
+    for (int o = 0; o < 32; ++o) {
+        float a = W.b1[o];
+#pragma unroll
+        for (int i = 0; i < 10; ++i) a = fmaf(W.w1[o][i], x[i], a);
+        h1[o] = fmaxf(a, 0.f);
+    }
+#pragma unroll
+    for (int o = 0; o < 16; ++o) {
+        float a = W.b2[o];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) a = fmaf(W.w2[o][i], h1[i], a);
+        h2[o] = fmaxf(a, 0.f);
+    }
+#pragma unroll
+    for (int o = 0; o < 3; ++o) {
+        float a = W.b3[o];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a = fmaf(W.w3[o][i], h2[i], a);
+        rgb[3 * (size_t)r + o] = 1.0f / (1.0f + expf(-a));
+    }
+}
+
 extern "C" {
+
+noit_status noit_infer_dfaoit(noit_ctx* ctx, const float* host_w, int32_t count, const float* features,
+                              uint32_t n, float* rgb, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_infer_dfaoit: ctx is NULL");
+    if (!host_w) return noit_fail(ctx, NOIT_ERR_NULL, "noit_infer_dfaoit: host_w is NULL");
+    if (count != NOIT_DFAOIT_PARAMS)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_infer_dfaoit: count %d != 931 (P:97-104)", count);
+    if (n == 0) return NOIT_OK;
+    if (!features || !rgb) return noit_fail(ctx, NOIT_ERR_NULL, "noit_infer_dfaoit: NULL buffer");
+    MlpWeights10 w;
+    memcpy(&w, host_w, sizeof w);
+    infer10_kernel<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(w, features, n, rgb);
+    ctx->launches += 1;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    return NOIT_OK;
+}
 
 noit_status noit_build_features(noit_ctx* ctx, const noit_fragbuf* fb, const noit_layers* out,
                                 void* stream)

@@ -138,6 +138,20 @@ def test_infer(noit, precision):
     assert ctx.infer(torch.empty((0, 5), device="cuda")).shape == (0, 3)
 
 
+def test_infer_dfaoit_width(noit):
+    """NEXT-4: the comparison system's 10 -> 32 -> 16 -> 3 sigmoid network (931 parameters)."""
+    from test_oracle_pins import _weights931
+    rng = np.random.default_rng(14)
+    w = _weights931(5)
+    n = 10007
+    x = rng.random((n, 10)).astype(np.float32)
+    x[:, 9] = rng.integers(0, 129, n)
+    got = noit.Noit().infer_dfaoit(w, torch.from_numpy(x).cuda()).cpu().numpy()
+    assert np.max(np.abs(got.astype(np.float64) - oracle.infer10(w, x))) <= 1e-5     # outputs in (0, 1)
+    with pytest.raises(noit.NoitError):
+        noit.Noit().infer_dfaoit(w[:771], torch.from_numpy(x).cuda())
+
+
 # -------------------------------------------------------------------------------------------
 # S1-S5 fused
 # -------------------------------------------------------------------------------------------
