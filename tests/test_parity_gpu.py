@@ -196,6 +196,26 @@ def test_resolve_dense_tiles(noit, dtype, lo, hi):
     check_resolve(noit, fbh, w, 1, got)
 
 
+@pytest.mark.parametrize("block", range(4))
+def test_resolve_random_stress(noit, block):
+    """48 small random frames: odd sizes (P not a multiple of 32, F not a multiple of 4), every list
+    length regime (empty .. far above the 128 cap: the cold global path), both colour formats and
+    weight precisions, exact depth ties."""
+    rng = np.random.default_rng(1000 + block)
+    for _ in range(12):
+        W, H = int(rng.integers(1, 90)), int(rng.integers(1, 30))
+        max_n = int(rng.choice([1, 3, 12, 40, 130, 300]))
+        dtype = np.float16 if rng.random() < 0.6 else np.float32
+        precision = int(rng.integers(0, 2))
+        heavy = (int(rng.integers(1, 6)), int(rng.choice([200, 700, 1700]))) if rng.random() < 0.4 else None
+        fbh = random_fb(rng, W, H, max_n, dtype, tie_frac=float(rng.choice([0.0, 0.3, 0.9])),
+                        empty_frac=float(rng.choice([0.0, 0.2, 0.7])), heavy=heavy)
+        w = noit_scenes.mlp_weights(int(rng.integers(0, 1000)))
+        ctx = noit.Noit(w, precision)
+        got = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
+        check_resolve(noit, fbh, w, precision, got)
+
+
 def test_resolve_empty_and_single_output(noit):
     w = noit_scenes.mlp_weights(0)
     ctx = noit.Noit(w, 0)
