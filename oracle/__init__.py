@@ -103,7 +103,8 @@ def build_features(fb) -> dict:
 
 
 def resolve(fb, weights_eff, background, half=None, quarter=None, cell_level=None,
-            level_to_lod=(2, 1, 0, 0), pixel_list=None, tail_override=None, out=None) -> dict:
+            level_to_lod=(2, 1, 0, 0), pixel_list=None, tail_override=None, out=None,
+            background_image=None) -> dict:
     """S1-S5 (+S7 with cell_level, +S9 with pixel_list).  `out` lets S9 write into existing
     arrays (pixels not in the list stay untouched)."""
     P = fb.width * fb.height
@@ -125,7 +126,9 @@ def resolve(fb, weights_eff, background, half=None, quarter=None, cell_level=Non
              _p(None if weights_eff is None else _chk(weights_eff, np.float32, 771)),
              _p(tail_override), _p(bg), _p(pixel_list),
              C.c_uint32(0 if pixel_list is None else pixel_list.size),
-             _p(out["trans"]), _p(out["final"]), _p(out["depth1"])]
+             _p(out["trans"]), _p(out["final"]), _p(out["depth1"]),
+             _p(None if background_image is None else _chk(np.ascontiguousarray(background_image, np.float32),
+                                                           np.float32, 4 * P))]
     rc = lib().oracle_resolve(*args)
     assert rc == 0, rc
     return out

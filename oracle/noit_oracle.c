@@ -417,7 +417,8 @@ int32_t oracle_resolve(int32_t width, int32_t height, const uint32_t *offsets, c
                        const uint8_t *cell_level, const uint8_t *level_to_lod,
                        const float *weights, const float *tail_override, const float *background,
                        const uint32_t *pixel_list, uint32_t pixel_count,
-                       float *out_trans, float *out_final, float *out_depth1)
+                       float *out_trans, float *out_final, float *out_depth1,
+                       const float *background_image /* [P][4] per-pixel C_b (A11, NEXT-4) or NULL */)
 {
     frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
     frag_view hb = {hw, hh, hoff, hdepth, hrgba, color_fmt};
@@ -435,12 +436,13 @@ int32_t oracle_resolve(int32_t width, int32_t height, const uint32_t *offsets, c
             level = cell_level[(y / 8) * cells_x + (x / 8)];
             lod = level_to_lod[level];
         }
+        const float *bgp = background_image ? background_image + 4 * p : background;
         if (lod == 0)
-            resolve_pixel_full(&fb, p, weights, tail_override, background, out_trans, out_final,
+            resolve_pixel_full(&fb, p, weights, tail_override, bgp, out_trans, out_final,
                                out_depth1);
         else
             resolve_pixel_coarse(&fb, lod == 1 ? &hb : &qb, 1 << lod, 64 >> level, x, y, weights,
-                                 background, out_trans, out_final, out_depth1);
+                                 bgp, out_trans, out_final, out_depth1);
     }
     return 0;
 }

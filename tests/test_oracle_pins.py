@@ -945,3 +945,25 @@ def test_infer10_vs_numpy_and_parameter_count():
     z = np.zeros(931, np.float32)
     z[928:] = [0.0, 1.0, -2.0]                             # zero weights: sigmoid of the bias
     assert close(oracle.infer10(z, x)[0], 1 / (1 + np.exp(-np.array([0.0, 1.0, -2.0]))), 1e-6, 1e-7)
+
+
+# -------------------------------------------------------------------------------------------
+# NEXT-4: per-pixel background (Eq. 4's last term with C_b varying over the image)
+# -------------------------------------------------------------------------------------------
+def test_per_pixel_background_closed_form():
+    rng = np.random.default_rng(70)
+    W, H = 23, 9
+    counts = rng.integers(0, 7, W * H)
+    F = int(counts.sum())
+    fb = make_fb(counts, rng.uniform(0.05, 0.95, F), rng.uniform(0, 1, (F, 4)).astype(np.float32), W, H)
+    w = oracle.effective_weights(noit_scenes.mlp_weights(9), 0)
+    bgi = rng.random((W * H, 4)).astype(np.float32)
+    out = oracle.resolve(fb, w, (9.0, 9.0, 9.0), background_image=bgi)    # the constant is ignored
+    # Eq. 4: C_p - C_t = prod(1 - a_i) C_b, pixel by pixel; the transparency result does not move
+    assert np.allclose(out["final"][:, :3] - out["trans"][:, :3], out["trans"][:, 3:4] * bgi[:, :3],
+                       rtol=1e-5, atol=1e-6)
+    ref = oracle.resolve(fb, w, (0.2, 0.3, 0.4))
+    assert np.array_equal(out["trans"], ref["trans"])
+    const = np.tile(np.asarray([[0.2, 0.3, 0.4, 0.0]], np.float32), (W * H, 1))
+    same = oracle.resolve(fb, w, (0, 0, 0), background_image=const)
+    assert np.array_equal(same["final"], ref["final"])
