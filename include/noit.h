@@ -148,6 +148,8 @@ typedef struct {
     const uint32_t* pixel_count;     /* device scalar: entries of pixel_list to process        */
     float* out_trans; float* out_final; float* out_depth1;
     const float* pass_scales;        /* device {w, s_2, s_3}, or NULL                          */
+    const float* background_image;   /* device [P][4] per-pixel C_b (.xyz used; NEXT-4) or NULL:
+                                        replaces `background` in out_final; 16-byte aligned    */
 } noit_resolve_desc;
 noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* desc, void* stream);
 

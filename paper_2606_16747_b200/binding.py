@@ -48,7 +48,8 @@ class ResolveDescC(C.Structure):
                 ("cell_level", C.c_void_p), ("level_to_lod", C.c_uint8 * 4),
                 ("background", C.c_float * 3), ("pixel_list", C.c_void_p),
                 ("pixel_count", C.c_void_p), ("out_trans", C.c_void_p), ("out_final", C.c_void_p),
-                ("out_depth1", C.c_void_p), ("pass_scales", C.c_void_p)]
+                ("out_depth1", C.c_void_p), ("pass_scales", C.c_void_p),
+                ("background_image", C.c_void_p)]
 
 
 class QtParamsC(C.Structure):
@@ -216,12 +217,15 @@ class Noit:
     # ---- S1-S5 (+S7, +S9) ---------------------------------------------------------------
     def make_resolve_desc(self, fb, background, out_trans=None, out_final=None, out_depth1=None,
                           half=None, quarter=None, cell_level=None, level_to_lod=(2, 1, 0, 0),
-                          pixel_list=None, pixel_count=None, pass_scales=None):
+                          pixel_list=None, pixel_count=None, pass_scales=None,
+                          background_image=None):
         """Marshal once, launch many times (the returned object keeps its tensors alive)."""
         d = ResolveDescC()
         d.full = fb.c_struct()
         d.pass_scales = _ptr(pass_scales)
-        keep = [fb, half, quarter, cell_level, pixel_list, pixel_count, pass_scales, out_trans, out_final,
+        d.background_image = _ptr(background_image)
+        keep = [fb, half, quarter, cell_level, pixel_list, pixel_count, pass_scales, background_image,
+                out_trans, out_final,
                 out_depth1]
         if half is not None:
             hc = half.c_struct()

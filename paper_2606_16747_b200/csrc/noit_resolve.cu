@@ -57,6 +57,8 @@ static noit_status check_desc(noit_ctx* ctx, const noit_resolve_desc* d, const c
     if (!noit_aligned(d->out_trans, 16) || !noit_aligned(d->out_final, 16) ||
         !noit_aligned(d->out_depth1, 4))
         return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: out_trans/out_final need 16-byte alignment", who);
+    if (!noit_aligned(d->background_image, 16))
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: background_image needs 16-byte alignment", who);
     if ((d->pixel_list != nullptr) != (d->pixel_count != nullptr))
         return noit_fail(ctx, NOIT_ERR_NULL, "%s: pixel_list and pixel_count go together", who);
     if (d->pixel_list && d->cell_level)
@@ -109,6 +111,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
     A.depth = d->full.depth;
     A.rgba = d->full.rgba;
     memcpy(A.bg, d->background, sizeof A.bg);
+    A.bg_image = d->background_image;
     A.out_trans = d->out_trans;
     A.out_final = d->out_final;
     A.out_depth1 = d->out_depth1;
@@ -177,7 +180,8 @@ noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* d, void* stream
 noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve_host: ctx is NULL");
-    if (h && (h->cell_level || h->pixel_list || h->half || h->quarter))
+    if (h && (h->cell_level || h->pixel_list || h->half || h->quarter || h->pass_scales ||
+              h->background_image))
         return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "noit_resolve_host: plain resolve only");
     NOIT_TRY(check_desc(ctx, h, "noit_resolve_host"));
     cudaStream_t st = (cudaStream_t)stream;

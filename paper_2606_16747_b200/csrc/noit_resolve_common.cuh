@@ -10,6 +10,7 @@ struct ResolveArgs {
     const float* depth;
     const void* rgba;
     float bg[3];
+    const float* bg_image;         // per-pixel background [P][4] or NULL (NEXT-4)
     float* out_trans;
     float* out_final;
     float* out_depth1;
@@ -85,10 +86,13 @@ __device__ __forceinline__ void composite_store(const ResolveArgs& A, uint32_t p
     const float t_tot = t2 * t_tail;
     if (A.out_trans)
         __stcs(reinterpret_cast<float4*>(A.out_trans) + p, make_float4(ct_r, ct_g, ct_b, t_tot));
-    if (A.out_final)
+    if (A.out_final) {
+        float4 bg = make_float4(A.bg[0], A.bg[1], A.bg[2], 0.f);
+        if (A.bg_image) bg = __ldcs(reinterpret_cast<const float4*>(A.bg_image) + p);
         __stcs(reinterpret_cast<float4*>(A.out_final) + p,
-               make_float4(fmaf(t_tot, A.bg[0], ct_r), fmaf(t_tot, A.bg[1], ct_g),
-                           fmaf(t_tot, A.bg[2], ct_b), 1.f - t_tot));
+               make_float4(fmaf(t_tot, bg.x, ct_r), fmaf(t_tot, bg.y, ct_g), fmaf(t_tot, bg.z, ct_b),
+                           1.f - t_tot));
+    }
     if (A.out_depth1) __stcs(A.out_depth1 + p, d1);
 }
 #endif

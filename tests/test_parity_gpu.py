@@ -216,6 +216,21 @@ def test_resolve_random_stress(noit, block):
         check_resolve(noit, fbh, w, precision, got)
 
 
+def test_resolve_per_pixel_background(noit):
+    """NEXT-4: C_b varies over the image; the transparency result is unchanged."""
+    rng = np.random.default_rng(33)
+    fbh = random_fb(rng, 97, 31, 40, np.float16, heavy=(3, 300))
+    w = noit_scenes.mlp_weights(4)
+    ctx = noit.Noit(w, 1)
+    bgi = rng.random((fbh.num_pixels, 4)).astype(np.float32)
+    fb = noit.DeviceFragBuf.from_host(fbh)
+    got = ctx.resolve(fb, (9.0, 9.0, 9.0), background_image=torch.from_numpy(bgi).cuda())
+    ref = oracle.resolve(fbh, oracle.effective_weights(w, 1), (9.0, 9.0, 9.0), background_image=bgi)
+    check_resolve(noit, fbh, w, 1, got, ref=ref)
+    plain = ctx.resolve(fb, BG)
+    assert torch.equal(plain["trans"], got["trans"])
+
+
 def test_resolve_empty_and_single_output(noit):
     w = noit_scenes.mlp_weights(0)
     ctx = noit.Noit(w, 0)
