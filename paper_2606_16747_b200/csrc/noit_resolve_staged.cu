@@ -304,7 +304,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 {
     typedef typename Color<ColorT>::Packed Packed;
     constexpr uint32_t CB = Color<ColorT>::kBytes;
-    constexpr uint32_t kStageBytes = kCap * (4u + CB);   // per warp
+    // per warp; S9 reads global memory directly and allocates no stage (more CTAs per SM)
+    constexpr uint32_t kStageBytes = kMode == NOIT_RESOLVE_LIST ? 0u : kCap * (4u + CB);
     // fragments when the stage holds depths only / colours only; multiples of 4 because a copy
     // is rounded up to 4 fragments
     constexpr uint32_t kCapD = (kStageBytes / 4u) & ~3u;
@@ -321,6 +322,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     const uint32_t bar = smem_u32(reinterpret_cast<uint64_t*>(smem_raw + kWarpsPerCta * kStageBytes +
                                                               kWarpsPerCta * kScratchFloats * sizeof(float)) + warp);
     static_assert(kStageBytes % 16 == 0 && (kCap * 4u) % 16 == 0, "bulk copies need 16-byte aligned destinations");
+    static_assert(kMode != NOIT_RESOLVE_LIST || kStageBytes == 0, "S9 never touches the stage");
     if (lane == 0) {
         mbar_init(bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -677,8 +679,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 template <typename ColorT, int L, bool kMma, int kMode>
 static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
 {
-    const size_t smem = kWarpsPerCta * (size_t)kCap * (4u + Color<ColorT>::kBytes) +
-                        kWarpsPerCta * sizeof(uint64_t) + kWarpsPerCta * kScratchFloats * sizeof(float);
+    const size_t stage = kMode == NOIT_RESOLVE_LIST ? 0 : (size_t)kCap * (4u + Color<ColorT>::kBytes);
+    const size_t smem = kWarpsPerCta * stage + kWarpsPerCta * sizeof(uint64_t) +
+                        kWarpsPerCta * kScratchFloats * sizeof(float);
     static bool configured = false;                     // per instantiation
     if (!configured) {
         NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma, kMode>,
@@ -708,6 +711,10 @@ static noit_status launch_mode(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t
     // lanes per pixel: 4 for frames; 8 for the pixel list (scattered lists are latency-bound:
     // shorter per-lane chains, 4-pixel tiles keep every warp of the machine busy)
     constexpr int L = kMode == NOIT_RESOLVE_LIST ? 8 : 4;
+    // S9 is bound by the latency chain of its few scattered tiles, not by issue slots: the FFMA2
+    // MLP needs 40 registers fewer than the tensor-core one, which with no stage allocated
+    // gives 7 CTAs per SM instead of 4 and so fewer tiles in sequence per warp
+    if (kMode == NOIT_RESOLVE_LIST) return launch_staged<ColorT, L, false, kMode>(ctx, A, st);
     return mma ? launch_staged<ColorT, L, true, kMode>(ctx, A, st)
                : launch_staged<ColorT, L, false, kMode>(ctx, A, st);
 }
