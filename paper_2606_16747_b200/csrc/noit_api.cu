@@ -127,24 +127,26 @@ noit_status noit_set_weights(noit_ctx* ctx, const float* host_w, int32_t count, 
             auto at = [&](int idx) -> float& { return pk[((idx >> 2) * 32 + lane) * 4 + (idx & 3)]; };
             for (int j = 0; j < 4; ++j) {
                 at(2 * j) = w.w1[8 * j + g][t];
-                at(2 * j + 1) = t == 0 ? w.w1[8 * j + g][4] : 0.f;
-                at(8 + 2 * j) = w.b1[8 * j + 2 * t];
-                at(8 + 2 * j + 1) = w.b1[8 * j + 2 * t + 1];
+                at(2 * j + 1) = t == 0 ? w.w1[8 * j + g][4] : (t == 1 ? w.b1[8 * j + g] : 0.f);
             }
             for (int j = 0; j < 2; ++j) {
                 for (int sidx = 0; sidx < 4; ++sidx) {
-                    at(16 + 2 * (4 * j + sidx)) = w.w2[8 * j + g][8 * sidx + 2 * t];
-                    at(16 + 2 * (4 * j + sidx) + 1) = w.w2[8 * j + g][8 * sidx + 2 * t + 1];
+                    at(8 + 2 * (4 * j + sidx)) = w.w2[8 * j + g][8 * sidx + 2 * t];
+                    at(8 + 2 * (4 * j + sidx) + 1) = w.w2[8 * j + g][8 * sidx + 2 * t + 1];
                 }
-                at(32 + 2 * j) = w.b2[8 * j + 2 * t];
-                at(32 + 2 * j + 1) = w.b2[8 * j + 2 * t + 1];
+                for (int h = 0; h < 2; ++h) {
+                    at(24 + 4 * j + 2 * h) = w.b2[8 * j + 2 * t];
+                    at(24 + 4 * j + 2 * h + 1) = w.b2[8 * j + 2 * t + 1];
+                }
             }
             for (int sidx = 0; sidx < 2; ++sidx) {
-                at(36 + 2 * sidx) = g < 3 ? w.w3[g][8 * sidx + 2 * t] : 0.f;
-                at(36 + 2 * sidx + 1) = g < 3 ? w.w3[g][8 * sidx + 2 * t + 1] : 0.f;
+                at(32 + 2 * sidx) = g < 3 ? w.w3[g][8 * sidx + 2 * t] : 0.f;
+                at(32 + 2 * sidx + 1) = g < 3 ? w.w3[g][8 * sidx + 2 * t + 1] : 0.f;
             }
-            at(40) = 2 * t < 3 ? w.b3[2 * t] : 0.f;
-            at(41) = 2 * t + 1 < 3 ? w.b3[2 * t + 1] : 0.f;
+            for (int h = 0; h < 2; ++h) {
+                at(36 + 2 * h) = 2 * t < 3 ? w.b3[2 * t] : 0.f;
+                at(36 + 2 * h + 1) = 2 * t + 1 < 3 ? w.b3[2 * t + 1] : 0.f;
+            }
         }
         if (!ctx->d_mlp) NOIT_CUDA(ctx, cudaMalloc(&ctx->d_mlp, sizeof pk));
         NOIT_CUDA(ctx, cudaMemcpy(ctx->d_mlp, pk, sizeof pk, cudaMemcpyHostToDevice));

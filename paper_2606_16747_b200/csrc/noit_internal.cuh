@@ -222,10 +222,14 @@ __device__ __forceinline__ void mlp_forward_packed(const MlpWeightsT& W, const f
 // layer l's n-tile s is, register for register, the A fragment of layer l+1's k-step s once
 // the hidden units are re-labelled (A col t <-> C col 2t, A col t+4 <-> C col 2t+1); that
 // re-labelling lives in the packed weights (noit_set_weights), so layers chain with no shuffle.
-// Packed weights: 11 float4 per lane, chunk v of lane l at wp[v*32 + l] (g = l>>2, t = l&3):
-//   0-1 W1 B-frags (4 n-tiles x {k=t, k=t+4}), 2-3 b1 (4 n-tiles x {col 2t, 2t+1}),
-//   4-7 W2 B-frags ((n-tile j, k-step s) x 2), 8 b2, 9 W3 B-frags (2 k-steps x 2), 10 b3.
-#define NOIT_MMA_CHUNKS 11
+// The bias of layer 1 rides in the zero padding of its K = 8: feature column 5 is the constant 1
+// (hi = 1, lo = 0) and row 5 of the B operand is b1, so those chains start from C = 0; the biases
+// of layers 2 and 3 are stored as whole C fragments {b[2t], b[2t+1], b[2t], b[2t+1]}, which a
+// chain's first MMA reads in place (no register moves to assemble the quad).
+// Packed weights: 10 float4 per lane, chunk v of lane l at wp[v*32 + l] (g = l>>2, t = l&3):
+//   0-1 W1 B-frags (4 n-tiles x {k=t, k=t+4}; k=5 is b1), 2-5 W2 B-frags ((n-tile j, k-step s) x 2),
+//   6-7 b2 C-frags (n-tile j), 8 W3 B-frags (2 k-steps x 2), 9 b3 C-frag.
+#define NOIT_MMA_CHUNKS 10
 __device__ __forceinline__ void mma_tf32(float (&d)[4], const float (&a)[4], float b0, float b1,
                                          const float (&c)[4])
 {
@@ -274,13 +278,14 @@ __device__ __forceinline__ void mlp_forward_mma(const float4 (&wv)[NOIT_MMA_CHUN
         split_tf32(r1[t], ahi[1], alo[1]);
         split_tf32(t == 0 ? r0[4] : 0.f, ahi[2], alo[2]);
         split_tf32(t == 0 ? r1[4] : 0.f, ahi[3], alo[3]);
-        // layer 1: 4 n-tiles, K = 8 (5 features + zero padding)
+        if (t == 1) ahi[2] = ahi[3] = 1.0f;                   // column 5: the constant feature
+        // layer 1: 4 n-tiles, K = 8 (5 features + the constant + zero padding)
+        const float zero[4] = {0.f, 0.f, 0.f, 0.f};
         float h1hi[4][4], h1lo[4][4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const float bias[4] = {wf(8 + 2 * j), wf(8 + 2 * j + 1), wf(8 + 2 * j), wf(8 + 2 * j + 1)};
             float c[4];
-            mma_tf32(c, ahi, wf(2 * j), wf(2 * j + 1), bias);
+            mma_tf32(c, ahi, wf(2 * j), wf(2 * j + 1), zero);
             mma_tf32(c, alo, wf(2 * j), wf(2 * j + 1), c);
             c_to_a(c, h1hi[j], h1lo[j]);
         }
@@ -288,21 +293,25 @@ __device__ __forceinline__ void mlp_forward_mma(const float4 (&wv)[NOIT_MMA_CHUN
         float h2hi[2][4], h2lo[2][4];
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-            float c[4] = {wf(32 + 2 * j), wf(32 + 2 * j + 1), wf(32 + 2 * j), wf(32 + 2 * j + 1)};
+            const float bias[4] = {wv[6 + j].x, wv[6 + j].y, wv[6 + j].z, wv[6 + j].w};
+            float c[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                const float b0 = wf(16 + 2 * (4 * j + s)), b1 = wf(16 + 2 * (4 * j + s) + 1);
-                mma_tf32(c, h1hi[s], b0, b1, c);
+                const float b0 = wf(8 + 2 * (4 * j + s)), b1 = wf(8 + 2 * (4 * j + s) + 1);
+                if (s == 0) mma_tf32(c, h1hi[s], b0, b1, bias);
+                else mma_tf32(c, h1hi[s], b0, b1, c);
                 mma_tf32(c, h1lo[s], b0, b1, c);
             }
             c_to_a(c, h2hi[j], h2lo[j]);
         }
         // layer 3: 1 n-tile (3 outputs, padded to 8), 2 k-steps
-        float c[4] = {wf(40), wf(41), wf(40), wf(41)};
+        const float bias3[4] = {wv[9].x, wv[9].y, wv[9].z, wv[9].w};
+        float c[4];
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
-            mma_tf32(c, h2hi[s], wf(36 + 2 * s), wf(36 + 2 * s + 1), c);
-            mma_tf32(c, h2lo[s], wf(36 + 2 * s), wf(36 + 2 * s + 1), c);
+            if (s == 0) mma_tf32(c, h2hi[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), bias3);
+            else mma_tf32(c, h2hi[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), c);
+            mma_tf32(c, h2lo[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), c);
         }
 #pragma unroll
         for (int k = 0; k < 4; ++k) fout[mt][k] = fmaxf(c[k], 0.f);

@@ -339,13 +339,25 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // The first three tiles of a warp are static (warp id + k * warps): no atomic round trips at
     // start-up; the counter hands out the tiles after those.
     const uint32_t n_warps = gridDim.x * kWarpsPerCta, warp_id = blockIdx.x * kWarpsPerCta + warp;
+    // (ptxas warp-aggregates an atomic whose address and addend are uniform -- vote, leader
+    // election, and a SHFL of the result right behind the ATOMG, which stalls the warp for the
+    // whole round trip -- even for inline PTX under `if (lane == 0)`.  The addend below is
+    // laneid + 1 under the predicate laneid == 0: not uniform to ptxas, so the atomic stays a
+    // plain predicated ATOMG and nothing waits for it until the broadcast a tile later.)
     auto fetch_raw = [&]() -> uint32_t {
         uint32_t t = 0;
-        if (lane == 0) {
-            asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(A.tile_counter) : "memory");
-            t += 3u * n_warps;
-        }
-        return t;
+        asm volatile("{\n"
+                     ".reg .pred p;\n"
+                     ".reg .u32 l, inc;\n"
+                     "mov.u32 l, %%laneid;\n"
+                     "setp.eq.u32 p, l, 0;\n"
+                     "add.u32 inc, l, 1;\n"
+                     "@p atom.global.add.u32 %0, [%1], inc;\n"
+                     "}\n"
+                     : "+r"(t)
+                     : "l"(A.tile_counter)
+                     : "memory");
+        return lane == 0 ? t + 3u * n_warps : 0u;
     };
     // S9 (kMode LIST): "tile" t = entries [t*32/L, (t+1)*32/L) of the pixel list; the lists of a
     // tile are not contiguous, so such tiles always take the global path.
