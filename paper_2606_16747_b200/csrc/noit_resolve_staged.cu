@@ -404,20 +404,25 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // caller has made sure nobody still reads the old contents.  The bulk copies never read
     // past the arrays: the last < 4 fragments of the frame are copied by lanes.
     bool pend = false;                                   // warp-uniform: a bulk copy is in flight
-    auto issue_fill = [&](float* dst_d, Packed* dst_c, uint32_t fs, uint32_t fe) {
+    // (which of the two arrays is copied is a literal at every call site: testing the shared-memory
+    // pointers against NULL instead costs a generic-address conversion per test)
+    auto issue_fill = [&](const bool has_d, const bool has_c, float* dst_d, Packed* dst_c, uint32_t fs,
+                          uint32_t fe) {
         __syncwarp();
         uint32_t n4 = (fe - fs + 3u) & ~3u;
-        if (fs + n4 > A.F) n4 = (A.F - fs) & ~3u;
+        if (fs + n4 > A.F) {                             // the frame's last tile only
+            n4 = (A.F - fs) & ~3u;
+            const uint32_t rem = fe - fs > n4 ? fe - fs - n4 : 0u;
+            if ((uint32_t)lane < rem) {
+                if (has_d) dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
+                if (has_c) dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
+            }
+        }
         if (lane == 0 && n4) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            mbar_expect_tx(bar, n4 * ((dst_d ? 4u : 0u) + (dst_c ? CB : 0u)));
-            if (dst_d) bulk_g2s(smem_u32(dst_d), A.depth + fs, n4 * 4u, bar);
-            if (dst_c) bulk_g2s(smem_u32(dst_c), g_rgba + fs, n4 * CB, bar);
-        }
-        const uint32_t rem = fe - fs > n4 ? fe - fs - n4 : 0u;
-        if ((uint32_t)lane < rem) {
-            if (dst_d) dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
-            if (dst_c) dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
+            mbar_expect_tx(bar, n4 * ((has_d ? 4u : 0u) + (has_c ? CB : 0u)));
+            if (has_d) bulk_g2s(smem_u32(dst_d), A.depth + fs, n4 * 4u, bar);
+            if (has_c) bulk_g2s(smem_u32(dst_c), g_rgba + fs, n4 * CB, bar);
         }
         pend = n4 != 0;
     };
@@ -455,14 +460,14 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         const uint32_t fs = tb & ~3u;
         if (te <= tb) return;
         if (depth_only_tile && te - fs <= kCapD) {
-            issue_fill(sD, nullptr, fs, te);
+            issue_fill(true, false, sD, nullptr, fs, te);
         } else if (te - fs <= kCap) {
-            issue_fill(sD, sC2, fs, te);
+            issue_fill(true, true, sD, sC2, fs, te);
         } else {
             uint32_t B[L + 1], bk;
             if (!round_bounds(a, te, B)) return;
             chunk_end(B, 0, kCapD, bk);
-            if (bk > B[0]) issue_fill(sD, nullptr, fs, bk);
+            if (bk > B[0]) issue_fill(true, false, sD, nullptr, fs, bk);
         }
     };
 
@@ -567,7 +572,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                         uint32_t bk;
                         const int k = chunk_end(B, r, kCapD, bk);
                         const uint32_t base = B[r] & ~3u;
-                        if (r > 0 && bk > B[r]) issue_fill(sD, nullptr, base, bk);   // r == 0: first_fill
+                        if (r > 0 && bk > B[r]) issue_fill(true, false, sD, nullptr, base, bk);   // r == 0: first_fill
                         wait_fill();
                         Dv = sD - base;
                         staged_to = k;
@@ -587,7 +592,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                         uint32_t bk;
                         const int k = chunk_end(B, r, kCapC, bk);
                         const uint32_t base = B[r] & ~3u;
-                        if (bk > B[r]) issue_fill(nullptr, sC, base, bk);
+                        if (bk > B[r]) issue_fill(false, true, nullptr, sC, base, bk);
                         wait_fill();
                         Cv = sC - base;
                         if (q >= r && q < k) {           // owners of the chunk's rounds
