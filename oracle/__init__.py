@@ -254,3 +254,29 @@ def reproject(width, height, M, depth_threshold, background, prev_trans, prev_de
     out["reject_count"] = int(cnt.value)
     out["reject_list"] = out["reject_list"][:cnt.value].copy()
     return out
+
+
+def reproject_bilinear(width, height, M, depth_threshold, background, prev_trans, prev_depth,
+                       cur_depth, out_trans=None, out_depth=None, out_final=None) -> dict:
+    """O8b (A28): O8 with a bilinear fetch of the previous result where all four taps pass the
+    disocclusion test; `filtered` marks those pixels."""
+    P = width * height
+    M = _chk(np.ascontiguousarray(M, np.float32).reshape(-1), np.float32, 16)
+    bg = np.asarray(background, np.float32)
+    out = dict(trans=np.zeros((P, 4), np.float32) if out_trans is None else out_trans,
+               depth=np.zeros(P, np.float32) if out_depth is None else out_depth,
+               final=np.zeros((P, 4), np.float32) if out_final is None else out_final,
+               accept=np.zeros(P, np.uint8), reject_list=np.zeros(P, np.uint32),
+               filtered=np.zeros(P, np.uint8))
+    cnt = C.c_uint32(0)
+    rc = lib().oracle_reproject_bilinear(C.c_int32(width), C.c_int32(height), _p(M),
+                                         C.c_float(depth_threshold), _p(bg),
+                                         _p(_chk(prev_trans, np.float32, 4 * P)),
+                                         _p(_chk(prev_depth, np.float32, P)),
+                                         _p(_chk(cur_depth, np.float32, P)), _p(out["trans"]),
+                                         _p(out["depth"]), _p(out["final"]), _p(out["accept"]),
+                                         _p(out["reject_list"]), C.byref(cnt), _p(out["filtered"]))
+    assert rc == 0
+    out["reject_count"] = int(cnt.value)
+    out["reject_list"] = out["reject_list"][:cnt.value].copy()
+    return out

@@ -899,6 +899,105 @@ int32_t oracle_reproject(int32_t width, int32_t height, const float *M, float de
     return 0;
 }
 
+/* O8b (NEXT-4, SURVEY 8(f) rank 4 "bilinear-filtered reprojection"; reading A28).  The paper
+ * itself fetches the nearest pixel; this variant differs from O8 only in the fetch of
+ * the previous result:
+ *   - the transform, the nearest previous pixel q, the on-screen test and the disocclusion test
+ *     |prev_depth[q] - d_e| <= tau are O8's, unchanged, so accept / reject_list / out_depth are
+ *     identical to O8's;
+ *   - with (u, v) the continuous previous-frame position (pixel centres at +0.5), the four taps
+ *     are x0 = floor(u - 0.5), x1 = x0 + 1 (both clamped to the image), same in y, with weights
+ *     wx = (u - 0.5) - floor(u - 0.5), wy likewise;
+ *   - the filtered value is used iff ALL FOUR taps pass the disocclusion test against d_e
+ *     (no blending across a depth discontinuity); otherwise the nearest pixel is kept (O8);
+ *   - fp32 in one fixed order: top = fma(wx, t01 - t00, t00), bot = fma(wx, t11 - t10, t10),
+ *     out = fma(wy, bot - top, top), per channel of (C_t, T_tot).
+ * Pins (tests/test_oracle_pins.py): whole-pixel shifts reduce to O8 bit for bit; a constant image
+ * stays constant; a dyadic linear ramp is reproduced exactly at a quarter-pixel shift; a depth
+ * edge falls back to O8 for exactly the pixels whose 2x2 footprint straddles it.               */
+int32_t oracle_reproject_bilinear(int32_t width, int32_t height, const float *M,
+                                  float depth_threshold, const float *background,
+                                  const float *prev_trans, const float *prev_depth,
+                                  const float *cur_depth, float *out_trans, float *out_depth,
+                                  float *out_final, uint8_t *accept, uint32_t *reject_list,
+                                  uint32_t *reject_count, uint8_t *filtered)
+{
+    uint32_t nrej = 0;
+    float fW = (float)width, fH = (float)height;
+    float inv_w = 1.0f / fW, inv_h = 1.0f / fH;
+    for (int y = 0; y < height; ++y)
+        for (int x = 0; x < width; ++x) {
+            size_t p = (size_t)y * width + x;
+            float xn = fmaf(2.0f * ((float)x + 0.5f), inv_w, -1.0f);
+            float yn = fmaf(2.0f * ((float)y + 0.5f), inv_h, -1.0f);
+            float d = cur_depth[p];
+            float c[4];
+            for (int k = 0; k < 4; ++k)
+                c[k] = fmaf(M[4 * k + 0], xn,
+                            fmaf(M[4 * k + 1], yn, fmaf(M[4 * k + 2], d, M[4 * k + 3])));
+            int ok = c[3] > 0.0f;
+            float d_e = 0.0f, u = 0.0f, v = 0.0f;
+            size_t q = 0;
+            if (ok) {
+                float xp = c[0] / c[3], yp = c[1] / c[3];
+                d_e = c[2] / c[3];
+                u = (xp + 1.0f) * 0.5f * fW;
+                v = (yp + 1.0f) * 0.5f * fH;
+                float fx = floorf(u), fy = floorf(v);
+                ok = (fx >= 0.0f) && (fx < fW) && (fy >= 0.0f) && (fy < fH);
+                if (ok) {
+                    q = (size_t)(int)fy * width + (size_t)(int)fx;
+                    ok = fabsf(prev_depth[q] - d_e) <= depth_threshold;
+                }
+            }
+            if (filtered) filtered[p] = 0;
+            if (ok) {
+                float t[4];
+                for (int k = 0; k < 4; ++k) t[k] = prev_trans[4 * q + k];
+                /* the 2x2 footprint around (u - 0.5, v - 0.5) */
+                float ub = u - 0.5f, vb = v - 0.5f;
+                float x0f = floorf(ub), y0f = floorf(vb);
+                float wx = ub - x0f, wy = vb - y0f;
+                int x0 = (int)x0f, y0 = (int)y0f, x1 = x0 + 1, y1 = y0 + 1;
+                if (x0 < 0) x0 = 0;
+                if (x1 > width - 1) x1 = width - 1;
+                if (y0 < 0) y0 = 0;
+                if (y1 > height - 1) y1 = height - 1;
+                size_t q00 = (size_t)y0 * width + x0, q01 = (size_t)y0 * width + x1;
+                size_t q10 = (size_t)y1 * width + x0, q11 = (size_t)y1 * width + x1;
+                int all4 = fabsf(prev_depth[q00] - d_e) <= depth_threshold &&
+                           fabsf(prev_depth[q01] - d_e) <= depth_threshold &&
+                           fabsf(prev_depth[q10] - d_e) <= depth_threshold &&
+                           fabsf(prev_depth[q11] - d_e) <= depth_threshold;
+                if (all4) {
+                    for (int k = 0; k < 4; ++k) {
+                        float t00 = prev_trans[4 * q00 + k], t01 = prev_trans[4 * q01 + k];
+                        float t10 = prev_trans[4 * q10 + k], t11 = prev_trans[4 * q11 + k];
+                        float top = fmaf(wx, t01 - t00, t00);
+                        float bot = fmaf(wx, t11 - t10, t10);
+                        t[k] = fmaf(wy, bot - top, top);
+                    }
+                    if (filtered) filtered[p] = 1;
+                }
+                for (int k = 0; k < 4; ++k) out_trans[4 * p + k] = t[k];
+                if (out_depth) out_depth[p] = d_e;
+                if (out_final) {
+                    for (int k = 0; k < 3; ++k)
+                        out_final[4 * p + k] =
+                            (float)((double)t[k] + (double)t[3] * (double)background[k]);
+                    out_final[4 * p + 3] = (float)(1.0 - (double)t[3]);
+                }
+                if (accept) accept[p] = 1;
+            } else {
+                if (accept) accept[p] = 0;
+                if (reject_list) reject_list[nrej] = (uint32_t)p;
+                ++nrej;
+            }
+        }
+    if (reject_count) *reject_count = nrej;
+    return 0;
+}
+
 int32_t oracle_num_threads(void)
 {
     int n = 1;

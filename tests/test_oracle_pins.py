@@ -590,6 +590,92 @@ def test_reproject_depth_threshold_and_w_sign():
     assert not oracle.reproject(W, H, M, tau, BG, trans, prev, cur)["accept"].any()
 
 
+# ---- O8b (NEXT-4, A28): bilinear-filtered reprojection ---------------------------------------
+def _shift_matrix(W, H, sx, sy):
+    M = np.eye(4)
+    M[0, 3] = 2.0 * sx / W              # previous position = current position + (sx, sy) pixels
+    M[1, 3] = 2.0 * sy / H
+    return M
+
+
+def test_reproject_bilinear_whole_pixel_shift_is_nearest():
+    """wx = wy = 0: the filtered fetch IS the nearest fetch, bit for bit (and identity camera)."""
+    rng = np.random.default_rng(40)
+    W, H = 128, 64
+    trans, _ = random_frame(rng, W, H)
+    flat = np.full(W * H, 0.5, np.float32)
+    for (kx, ky) in ((0, 0), (3, 0), (-5, 2), (0, -7)):
+        M = _shift_matrix(W, H, kx, ky)
+        a = oracle.reproject(W, H, M, 1e-3, BG, trans, flat, flat)
+        b = oracle.reproject_bilinear(W, H, M, 1e-3, BG, trans, flat, flat)
+        for k in ("trans", "depth", "final", "accept"):
+            assert np.array_equal(a[k], b[k]), k
+        assert a["reject_count"] == b["reject_count"]
+        assert set(a["reject_list"].tolist()) == set(b["reject_list"].tolist())
+        assert np.array_equal(b["filtered"], b["accept"])      # flat depth: all four taps pass
+
+
+def test_reproject_bilinear_constant_image_stays_constant():
+    rng = np.random.default_rng(41)
+    W, H = 96, 40
+    const = np.array([0.3, 0.55, 0.125, 0.7], np.float32)
+    trans = np.tile(const, (W * H, 1))
+    flat = np.full(W * H, 0.25, np.float32)
+    for _ in range(4):
+        sx, sy = rng.uniform(-3, 3, 2)
+        r = oracle.reproject_bilinear(W, H, _shift_matrix(W, H, sx, sy), 1e-3, BG, trans, flat, flat)
+        acc = r["accept"].astype(bool)
+        assert acc.any() and np.array_equal(r["trans"][acc], trans[acc])
+
+
+def test_reproject_bilinear_reproduces_a_dyadic_ramp_exactly():
+    """Bilinear interpolation is exact on a*x + b*y + c; with dyadic coefficients and a dyadic
+    sub-pixel shift every fp32 step is exact, so the closed form must match bit for bit.  The
+    x / y weights differ (0.25 / 0.75) and so do the slopes: a swapped axis, an inverted weight
+    or a wrong tap order all fail."""
+    W, H = 128, 64
+    kx, ky, fx, fy = 2, -3, 0.25, 0.75
+    yy, xx = np.mgrid[0:H, 0:W].astype(np.float64)
+    coef = [(3, 5, 7), (-2, 1, 400), (1, -4, 300), (6, 2, 1)]
+    trans = np.stack([(a * xx + b * yy + c) / 1024.0 for (a, b, c) in coef], -1)
+    trans = trans.reshape(-1, 4).astype(np.float32)
+    flat = np.full(W * H, 0.5, np.float32)
+    r = oracle.reproject_bilinear(W, H, _shift_matrix(W, H, kx + fx, ky + fy), 1e-3, BG, trans,
+                                  flat, flat)
+    out = r["trans"].reshape(H, W, 4)
+    # sample position in previous pixel-index units: (x + kx + fx, y + ky + fy)
+    px, py = xx + kx + fx, yy + ky + fy
+    interior = (px >= 0) & (px <= W - 1) & (py >= 0) & (py <= H - 1)
+    assert interior.sum() > 0.8 * W * H
+    assert r["accept"].reshape(H, W)[interior].all() and r["filtered"].reshape(H, W)[interior].all()
+    for k, (a, b, c) in enumerate(coef):
+        want = ((a * px + b * py + c) / 1024.0).astype(np.float32)
+        assert np.array_equal(out[..., k][interior], want[interior]), k
+
+
+def test_reproject_bilinear_keeps_nearest_across_a_depth_edge():
+    """A28: a 2x2 footprint that straddles a depth discontinuity is not blended."""
+    rng = np.random.default_rng(42)
+    W, H, xs, tau = 64, 16, 23, 1e-3
+    trans, _ = random_frame(rng, W, H)
+    depth = np.where(np.arange(W)[None, :] < xs, 0.3, 0.7).astype(np.float32) * np.ones((H, 1), np.float32)
+    depth = depth.reshape(-1)
+    M = _shift_matrix(W, H, 0.25, 0.0)          # nearest pixel = the pixel itself, taps x and x+1
+    a = oracle.reproject(W, H, M, tau, BG, trans, depth, depth)
+    b = oracle.reproject_bilinear(W, H, M, tau, BG, trans, depth, depth)
+    assert a["accept"].all() and b["accept"].all()
+    filt = b["filtered"].reshape(H, W).astype(bool)
+    want = np.ones((H, W), bool)
+    want[:, xs - 1] = False                     # taps xs-1 (0.3) and xs (0.7)
+    assert np.array_equal(filt, want)
+    A, B, T = a["trans"].reshape(H, W, 4), b["trans"].reshape(H, W, 4), trans.reshape(H, W, 4)
+    assert np.array_equal(B[:, xs - 1], A[:, xs - 1])           # nearest kept, bit copy
+    x1 = np.minimum(np.arange(W) + 1, W - 1)
+    lerp = 0.75 * T.astype(np.float64) + 0.25 * T[:, x1].astype(np.float64)
+    assert close(B[filt], lerp[filt], 1e-6, 1e-7)
+    assert np.array_equal(a["depth"], b["depth"])
+
+
 def test_fallback_covers_every_pixel_once(cfg1_scene):
     """O9: accepted U resolved = every pixel exactly once; tau_d < 0 => plain resolve bitwise."""
     fb = cfg1_scene.full
