@@ -357,6 +357,13 @@ def run_ours(args):
               "inference_time_saved_by_5_features": 1.0 - t5 / t10,
               "quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
               "quadtree_balance": timed(lambda: ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal))}
+    # NEXT-4 (O8b): the step's reprojection with the bilinear fetch, into buffers of its own
+    rpb = {"o": None}
+    def run_rp(filt):
+        rpb["o"] = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"],
+                                 out=rpb["o"], filter=filt)
+    extras["reproject_nearest"] = timed(lambda: run_rp("nearest"))
+    extras["reproject_bilinear"] = timed(lambda: run_rp("bilinear"))
     clocks = sampler.stop() if rank == 0 else None
     rejected = int(rp["reject_count"].item())
     hist = bal["hist"].cpu().numpy().view(np.uint32).tolist()

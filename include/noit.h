@@ -232,7 +232,15 @@ noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32_t height, 
  * copy), out_depth[p] = d_e, accept[p] = 1, out_final[p] = (C_t + T_tot C_b, 1 - T_tot).
  * Rejected: accept[p] = 0, p appended to reject_list (order unspecified), outputs untouched.
  * M = VP_prev * VP_cur^-1, row-major, column vectors.  out_depth/out_final/accept/reject_list
- * may be NULL; reject_count (required) is zeroed by the call.                                */
+ * may be NULL; reject_count (required) is zeroed by the call.
+ * filter (NEXT-4, O8b / A28): NOIT_REPROJECT_NEAREST is the paper's fetch
+ * (P:121).  NOIT_REPROJECT_BILINEAR changes only the value fetched for an ACCEPTED pixel: the
+ * 2x2 footprint of prev_trans around the continuous previous position (taps clamped to the
+ * image, weights wx, wy in fp32, top = fma(wx, t01 - t00, t00), bot likewise,
+ * out = fma(wy, bot - top, top)) where all four taps pass the disocclusion test against d_e,
+ * the nearest pixel elsewhere; accept, reject_list and out_depth are the same for both filters.
+ * Any other value: NOIT_ERR_FORMAT.                                                            */
+enum { NOIT_REPROJECT_NEAREST = 0, NOIT_REPROJECT_BILINEAR = 1 };
 typedef struct {
     int32_t width, height;
     float M[16];
@@ -242,6 +250,7 @@ typedef struct {
     float* out_trans; float* out_depth; float* out_final;
     uint8_t* accept;
     uint32_t* reject_list; uint32_t* reject_count;
+    int32_t filter;
 } noit_reproject_desc;
 noit_status noit_reproject(noit_ctx* ctx, const noit_reproject_desc* desc, void* stream);
 

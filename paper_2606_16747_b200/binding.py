@@ -67,7 +67,8 @@ class ReprojectDescC(C.Structure):
                 ("depth_threshold", C.c_float), ("background", C.c_float * 3),
                 ("prev_trans", C.c_void_p), ("prev_depth", C.c_void_p), ("cur_depth", C.c_void_p),
                 ("out_trans", C.c_void_p), ("out_depth", C.c_void_p), ("out_final", C.c_void_p),
-                ("accept", C.c_void_p), ("reject_list", C.c_void_p), ("reject_count", C.c_void_p)]
+                ("accept", C.c_void_p), ("reject_list", C.c_void_p), ("reject_count", C.c_void_p),
+                ("filter", C.c_int32)]
 
 
 _lib = None
@@ -350,7 +351,7 @@ class Noit:
 
     # ---- S8 ---------------------------------------------------------------------------
     def reproject(self, width, height, M, depth_threshold, background, prev_trans, prev_depth,
-                  cur_depth, out=None, stream=None):
+                  cur_depth, out=None, stream=None, filter="nearest"):
         import numpy as np
         P, dev = width * height, prev_trans.device
         out = dict(out) if out else {}
@@ -372,5 +373,6 @@ class Noit:
         d.out_trans, d.out_depth, d.out_final = _ptr(out["trans"]), _ptr(out["depth"]), _ptr(out["final"])
         d.accept, d.reject_list, d.reject_count = (_ptr(out["accept"]), _ptr(out["reject_list"]),
                                                    _ptr(out["reject_count"]))
+        d.filter = {"nearest": 0, "bilinear": 1}[filter] if isinstance(filter, str) else int(filter)
         self._check(self._L.noit_reproject(self._ctx, C.byref(d), _stream(stream)))
         return out

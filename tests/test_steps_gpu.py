@@ -175,6 +175,67 @@ def test_reproject_perspective_path(noit):
     assert ref["reject_count"] == W * H
 
 
+def check_reproject_bilinear(noit, W, H, M, thr, prev_t, prev_d, cur_d):
+    """NEXT-4 / O8b: same fixed-order fp32 on both sides -> every output bit-exact; accept,
+    reject list and depth equal the nearest filter's."""
+    ctx = noit.Noit()
+    dev = [torch.from_numpy(a).cuda() for a in (prev_t, prev_d, cur_d)]
+    got = ctx.reproject(W, H, M, thr, BG, *dev, filter="bilinear")
+    near = ctx.reproject(W, H, M, thr, BG, *dev)
+    ref = oracle.reproject_bilinear(W, H, M, thr, BG, prev_t, prev_d, cur_d)
+    acc = got["accept"].cpu().numpy()
+    assert np.array_equal(acc, ref["accept"])
+    assert np.array_equal(acc, near["accept"].cpu().numpy())
+    n = int(got["reject_count"].item())
+    assert n == ref["reject_count"]
+    assert np.array_equal(np.sort(u32(got["reject_list"])[:n]), np.sort(ref["reject_list"]))
+    m = acc.astype(bool)
+    assert np.array_equal(got["trans"].cpu().numpy()[m], ref["trans"][m])      # bit-exact lerps
+    assert np.array_equal(got["depth"].cpu().numpy()[m], ref["depth"][m])
+    close(got["final"].cpu().numpy()[m], ref["final"][m])
+    assert not got["trans"].cpu().numpy()[~m].any()
+    # where the footprint was not used the value is the nearest fetch, bit for bit
+    keep = m & (ref["filtered"] == 0)
+    assert np.array_equal(got["trans"].cpu().numpy()[keep], near["trans"].cpu().numpy()[keep])
+    return got, ref
+
+
+def test_reproject_bilinear_subpixel_shift_and_edges(noit):
+    rng = np.random.default_rng(23)
+    W, H = 333, 77                                                             # ragged sizes, clamped taps
+    prev_t, prev_d = rand_prev(rng, W, H)
+    flat = np.full(W * H, 0.5, np.float32)
+    for (sx, sy) in ((0.0, 0.0), (0.3, -0.6), (-2.25, 1.75), (5.5, 0.0)):
+        M = np.eye(4, dtype=np.float32)
+        M[0, 3], M[1, 3] = 2.0 * sx / W, 2.0 * sy / H
+        _, ref = check_reproject_bilinear(noit, W, H, M, 1e-3, prev_t, flat, flat)
+        assert ref["filtered"].sum() == ref["accept"].sum() > 0               # flat depth: all filtered
+        # random depths: most footprints straddle a "discontinuity" and keep the nearest pixel
+        _, ref = check_reproject_bilinear(noit, W, H, M, 0.2, prev_t, prev_d, prev_d)
+        if (sx, sy) != (0.0, 0.0):
+            f = ref["filtered"][ref["accept"].astype(bool)]
+            assert 0 < f.sum() < f.size
+    with pytest.raises(Exception):
+        noit.Noit().reproject(W, H, np.eye(4, dtype=np.float32), 1e-3, BG, torch.from_numpy(prev_t).cuda(),
+                              torch.from_numpy(flat).cuda(), torch.from_numpy(flat).cuda(), filter=7)
+
+
+def test_reproject_bilinear_perspective_path(noit):
+    rng = np.random.default_rng(24)
+    W, H = 640, 360
+    proj = noit_scenes.perspective(60.0, W / H, 0.1, 100.0)
+    vp0 = proj @ noit_scenes.view_matrix(np.zeros(3), 0.0, 0.0)
+    vp1 = proj @ noit_scenes.view_matrix(np.asarray([0.05, -0.02, 0.03]), 0.004, -0.003)
+    M = (vp0 @ np.linalg.inv(vp1)).astype(np.float32)
+    prev_t, _ = rand_prev(rng, W, H)
+    yy, xx = np.mgrid[0:H, 0:W]
+    prev_d = (0.97 + 0.02 * np.sin(xx / 50.0) * np.cos(yy / 40.0)).astype(np.float32).reshape(-1)
+    prev_d[rng.random(W * H) < 0.05] = 1.0
+    _, ref = check_reproject_bilinear(noit, W, H, M, 1e-3, prev_t, prev_d, prev_d)
+    acc = ref["accept"].astype(bool)
+    assert 0 < ref["filtered"][acc].sum() < acc.sum()
+
+
 def test_fallback_resolve_on_reject_list(noit):
     """S8 + S9: union of accepted and re-resolved pixels covers the frame exactly once; with a
     negative threshold everything is rejected and the frame equals the plain resolve (layer-1
