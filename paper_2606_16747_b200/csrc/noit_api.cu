@@ -75,6 +75,7 @@ void noit_destroy(noit_ctx* ctx)
     if (!ctx) return;
     cudaFree(ctx->d_counters);
     cudaFree(ctx->d_mlp);
+    cudaFree(ctx->d_tile_lod);
     cudaFree(ctx->d_coarse_g[0]);
     cudaFree(ctx->d_coarse_g[1]);
     cudaFree(ctx->d_stage);

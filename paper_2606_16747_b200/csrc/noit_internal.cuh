@@ -41,6 +41,8 @@ struct noit_ctx {
     int precision = 0;
     MlpWeights w;                    // effective weights, host copy (kernel argument source)
     MlpWeightsT wt;                  // the same weights, input-major (FFMA2 form)
+    uint8_t* d_tile_lod = nullptr;   // S7 per-tile mode: lod summary byte per 32-pixel tile
+    size_t tile_lod_cap = 0;
     void* d_mlp = nullptr;           // device copy of the packed tensor-core operands (bf16 path)
     uint64_t launches = 0;
     char err[512] = {0};

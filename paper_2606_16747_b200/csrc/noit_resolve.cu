@@ -8,8 +8,11 @@ noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int 
 
 // S7 pre-pass: G (10 values in 12 floats) of every coarse pixel whose leaf is resolved at that lod (self-contained
 // O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
-// One launch covers both coarse levels: blocks [0, blocks1) the half-res buffer (lod 1), the rest
-// the quarter-res buffer (lod 2).
+// One launch covers both coarse levels: blocks [0, blocks1) the half-res buffer (lod 1), blocks
+// [blocks1, blocks12) the quarter-res buffer (lod 2).  In the per-tile mode the blocks from
+// blocks12 on write the lod summary of the staged kernel's 32-pixel tiles (one thread per tile):
+// bit 0 = some pixel of the tile has lod > 0, bit 1 = every pixel does (pixels past the frame
+// count as coarse), so the tile loop reads one byte instead of a level per lane and two votes.
 struct CoarseLevel {
     int cw, ch;
     const uint32_t* offsets;
@@ -19,9 +22,28 @@ struct CoarseLevel {
 };
 template <typename ColorT>
 __global__ void __launch_bounds__(128)
-coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, int full_w,
-                const uint8_t* __restrict__ cell_level, uchar4 level_to_lod)
+coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, uint32_t blocks12, int full_w,
+                const uint8_t* __restrict__ cell_level, uchar4 level_to_lod, uint8_t* __restrict__ tile_lod,
+                uint32_t num_tiles, uint32_t P)
 {
+    if (blockIdx.x >= blocks12) {                         // lod summary of tile t (per-tile mode)
+        const uint32_t t = (blockIdx.x - blocks12) * blockDim.x + threadIdx.x;
+        if (t >= num_tiles) return;
+        const uint8_t l2l[4] = {level_to_lod.x, level_to_lod.y, level_to_lod.z, level_to_lod.w};
+        const uint32_t W = (uint32_t)full_w, cw8 = (W + 7u) >> 3;
+        uint32_t p = t * 32u;
+        const uint32_t end = min(p + 32u, P);
+        bool any = false, all = true;
+        while (p < end) {                                 // one step per 8x8 cell the tile crosses
+            const uint32_t y = p / W, x = p - y * W;
+            const int lod = l2l[cell_level[(size_t)(y >> 3) * cw8 + (x >> 3)] & 3];
+            any = any || lod > 0;
+            all = all && lod > 0;
+            p += min(8u - (x & 7u), W - x);
+        }
+        tile_lod[t] = (uint8_t)((any ? 1u : 0u) | ((any && all) ? 2u : 0u));
+        return;
+    }
     const bool second = blockIdx.x >= blocks1;
     const CoarseLevel lv = second ? lv2 : lv1;
     const int lod = second ? 2 : 1, r = 1 << lod;
@@ -153,13 +175,33 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
                                       ctx->d_coarse_g[lod - 1]};
             blocks[lod - 1] = (uint32_t)((cp + 127) / 128);
         }
-        if (blocks[0] + blocks[1]) {
+        // per-tile mode with no level mapped to a coarse lod: the frame is a plain resolve
+        if (d->cell_level && blocks[0] + blocks[1] == 0)
+            return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_ALL, st);
+        const uint32_t num_tiles = (A.P + 31u) / 32u;
+        uint32_t blocks_s = 0;
+        if (d->cell_level) {
+            if (ctx->tile_lod_cap < num_tiles) {
+                if (ctx->d_tile_lod) {
+                    NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+                    NOIT_CUDA(ctx, cudaFree(ctx->d_tile_lod));
+                    ctx->d_tile_lod = nullptr;
+                    ctx->tile_lod_cap = 0;
+                }
+                NOIT_CUDA(ctx, cudaMalloc(&ctx->d_tile_lod, num_tiles));
+                ctx->tile_lod_cap = num_tiles;
+            }
+            A.tile_lod = ctx->d_tile_lod;
+            blocks_s = (num_tiles + 127u) / 128u;
+        }
+        if (blocks[0] + blocks[1] + blocks_s) {
+            const uint32_t b12 = blocks[0] + blocks[1];
             if (fmt == NOIT_RGBA_F16)
-                coarse_g_kernel<__half><<<blocks[0] + blocks[1], 128, 0, st>>>(
-                    lv[0], lv[1], blocks[0], A.W, d->cell_level, l2l);
+                coarse_g_kernel<__half><<<b12 + blocks_s, 128, 0, st>>>(
+                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
             else
-                coarse_g_kernel<float><<<blocks[0] + blocks[1], 128, 0, st>>>(
-                    lv[0], lv[1], blocks[0], A.W, d->cell_level, l2l);
+                coarse_g_kernel<float><<<b12 + blocks_s, 128, 0, st>>>(
+                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
         }

@@ -20,6 +20,7 @@ struct ResolveArgs {
     // S7 / frame-global LOD (O7g)
     const float* pass_scales;      // device {w, s_2, s_3}: frame-global pass-2 / pass-3 lod
     const uint8_t* cell_level;
+    const uint8_t* tile_lod;        // per-tile mode: bit 0 mixed, bit 1 depth-only, per 32-pixel tile
     uint8_t level_to_lod[4];
     const float* coarse_g[2];      // G[10] per coarse pixel, lod 1 (half) and lod 2 (quarter)
     int32_t coarse_w[2], coarse_h[2];

@@ -400,6 +400,17 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)] & 3;
         return A.level_to_lod[level];
     };
+    // What the tile loop needs to know about a tile's lods: bit 0 = some pixel has lod > 0
+    // ("mixed": the epilogue looks at G), bit 1 = every pixel takes layer 2 AND the tail from a
+    // coarse buffer (only the depths are staged).  Per-tile mode: one byte per tile written by the
+    // pre-pass (tile_lod_summary in noit_resolve.cu) -- a level lookup per lane plus two votes per
+    // tile cost the mode 100 instructions per tile; frame-global mode: the same for every tile.
+    const uint32_t g_flags = (max(g_lod2, g_lod3) > 0 ? 1u : 0u) | ((g_lod2 > 0 && g_lod3 > 0) ? 3u : 0u);
+    auto tile_flags = [&](uint32_t tile) -> uint32_t {
+        if (kMode != NOIT_RESOLVE_ADAPTIVE) return 0u;
+        if (A.pass_scales) return g_flags;
+        return __ldg(A.tile_lod + (num_tiles - 1u - tile));
+    };
     // Issue the copy of fragments [fs, fe) (fs a multiple of 4 = 16 bytes) into the stage; the
     // caller has made sure nobody still reads the old contents.  The bulk copies never read
     // past the arrays: the last < 4 fragments of the frame are copied by lanes.
@@ -476,19 +487,14 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     uint32_t t_cur = warp_id;
     uint32_t raw_nxt = warp_id + n_warps, raw_nn = warp_id + 2u * n_warps;   // then two atomics in flight
     uint32_t o0 = 0, o1 = 0, pix = 0;
-    int lod = 0, level = 3;
     bool mixed = false;                                  // S7 / O7g: some pixel of the tile has lod > 0
     bool depth_only = false;                             // ... every pixel takes layer 2 AND tail coarse
-    // a lane whose pixel needs nothing but layer 1 from the full-resolution list
-    auto coarse_lane = [&](uint32_t pixel, int l) -> bool {
-        return pixel >= A.P || (A.pass_scales ? (g_lod2 > 0 && g_lod3 > 0) : l > 0);
-    };
     if (t_cur < num_tiles) {
         pix = lane_pixel(t_cur);
         load_offsets(pix, o0, o1);
-        lod = lane_lod(pix, level);
-        mixed = __any_sync(0xffffffffu, lod > 0);
-        depth_only = mixed && __all_sync(0xffffffffu, coarse_lane(pix, lod));
+        const uint32_t fl = tile_flags(t_cur);
+        mixed = (fl & 1u) != 0;
+        depth_only = (fl & 2u) != 0;
         first_fill(o0, o1, depth_only);
     }
     while (t_cur < num_tiles) {
@@ -496,11 +502,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         raw_nxt = raw_nn;
         raw_nn = fetch_raw();
         uint32_t no0 = 0, no1 = 0, npix = 0;
-        int nlod = 0, nlevel = 3;
+        uint32_t nflags = 0;
         if (t_nxt < num_tiles) {                         // lands while this tile runs
             npix = lane_pixel(t_nxt);
             load_offsets(npix, no0, no1);
-            nlod = lane_lod(npix, nlevel);
+            nflags = tile_flags(t_nxt);
         }
 
         Owned<ColorT> own;
@@ -625,9 +631,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
 #pragma unroll
             for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(A.mlp_packed + v * 32 + lane);
         }
-        // (the vote is taken here, not where the level was requested: it would wait for the load)
-        const bool nmixed = kMode == NOIT_RESOLVE_ADAPTIVE && __any_sync(0xffffffffu, nlod > 0);
-        const bool ndepth_only = nmixed && __all_sync(0xffffffffu, coarse_lane(npix, nlod));
+        const bool nmixed = (nflags & 1u) != 0, ndepth_only = (nflags & 2u) != 0;
         if (t_nxt < num_tiles) first_fill(no0, no1, ndepth_only);
         // ---- every lane now owns one pixel: features (O3), MLP (O4), composite (O5)
         uint32_t p = __shfl_sync(0xffffffffu, pix, (int)px_own);
@@ -679,7 +683,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             else mlp_forward_packed(W, xf, f);
             if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
-        pix = npix; lod = nlod; level = nlevel; mixed = nmixed; depth_only = ndepth_only;
+        pix = npix; mixed = nmixed; depth_only = ndepth_only;
         t_cur = t_nxt; o0 = no0; o1 = no1;
     }
     // the last warp to finish re-arms the counters for the next launch
