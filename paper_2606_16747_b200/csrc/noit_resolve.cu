@@ -205,7 +205,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
         }
-        return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_ADAPTIVE, st);
+        return noit_launch_resolve_staged(ctx, A, fmt, d->pass_scales ? NOIT_RESOLVE_GLOBAL : NOIT_RESOLVE_ADAPTIVE, st);
     }
     return noit_launch_resolve_staged(ctx, A, fmt, NOIT_RESOLVE_ALL, st);
 }

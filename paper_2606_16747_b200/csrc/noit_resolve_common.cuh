@@ -30,7 +30,9 @@ struct ResolveArgs {
     uint32_t* tile_counter;        // [0] next tile, [1] finished warps; self-resetting
 };
 
-enum { NOIT_RESOLVE_ALL = 0, NOIT_RESOLVE_LIST = 1, NOIT_RESOLVE_ADAPTIVE = 2 };
+// ADAPTIVE = per-tile lods from cell_level (S7); GLOBAL = frame-global lods from pass_scales (O7g):
+// separate instantiations, so neither carries the other's state in registers
+enum { NOIT_RESOLVE_ALL = 0, NOIT_RESOLVE_LIST = 1, NOIT_RESOLVE_ADAPTIVE = 2, NOIT_RESOLVE_GLOBAL = 3 };
 
 #ifdef __CUDACC__
 // lod > 0 pixel of S7 (O7): bilinear sample of G = [a2*C2 (3), a2, C_acc (3), A_tail, T_tail, N]

@@ -311,6 +311,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     constexpr uint32_t kCapD = (kStageBytes / 4u) & ~3u;
     constexpr uint32_t kCapC = (kStageBytes / CB) & ~3u;
     constexpr int PPR = 32 / L;
+    constexpr bool kGlobal = kMode == NOIT_RESOLVE_GLOBAL;              // frame-global lods (O7g)
+    constexpr bool kCoarse = kMode == NOIT_RESOLVE_ADAPTIVE || kGlobal;   // some pixels may read G
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned char* stage = smem_raw + warp * kStageBytes;
@@ -387,15 +389,15 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // do stages only its depths.
     // frame-global lods of pass 2 / pass 3 from the Eq. 2 scales (O7g, A27), decided here
     int g_lod2 = 0, g_lod3 = 0;
-    if (kMode == NOIT_RESOLVE_ADAPTIVE && A.pass_scales) {
+    if (kGlobal) {
         const float s2 = __ldg(A.pass_scales + 1), s3 = __ldg(A.pass_scales + 2);
         g_lod2 = s2 > 0.70710678f ? 0 : (s2 > 0.35355339f ? 1 : 2);
         g_lod3 = s3 > 0.70710678f ? 0 : (s3 > 0.35355339f ? 1 : 2);
     }
     auto lane_lod = [&](uint32_t pix, int& level) -> int {
         level = 3;
-        if (kMode != NOIT_RESOLVE_ADAPTIVE || pix >= A.P) return 0;
-        if (A.pass_scales) return max(g_lod2, g_lod3);
+        if (!kCoarse || pix >= A.P) return 0;
+        if (kGlobal) return max(g_lod2, g_lod3);
         const uint32_t y = pix / (uint32_t)A.W, x = pix - y * (uint32_t)A.W;
         level = A.cell_level[(size_t)(y >> 3) * ((A.W + 7) >> 3) + (x >> 3)] & 3;
         return A.level_to_lod[level];
@@ -407,8 +409,8 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // tile cost the mode 100 instructions per tile; frame-global mode: the same for every tile.
     const uint32_t g_flags = (max(g_lod2, g_lod3) > 0 ? 1u : 0u) | ((g_lod2 > 0 && g_lod3 > 0) ? 3u : 0u);
     auto tile_flags = [&](uint32_t tile) -> uint32_t {
-        if (kMode != NOIT_RESOLVE_ADAPTIVE) return 0u;
-        if (A.pass_scales) return g_flags;
+        if (!kCoarse) return 0u;
+        if (kGlobal) return g_flags;
         return __ldg(A.tile_lod + (num_tiles - 1u - tile));
     };
     // Issue the copy of fragments [fs, fe) (fs a multiple of 4 = 16 bytes) into the stage; the
@@ -529,7 +531,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             // every warp of the machine busy); lanes with lane % L == 0 own a pixel
             px_own = (uint32_t)(lane / L);
             own = tile_from_global<ColorT, L, 1>(lane, o0, o1, A.depth, g_rgba);
-        } else if (kMode == NOIT_RESOLVE_ADAPTIVE && depth_only && te - fs <= kCapD) {
+        } else if (kCoarse && depth_only && te - fs <= kCapD) {
             // ---- S7 / O7g tile whose 32 pixels all take layer 2 and the tail from a coarse buffer:
             // only layer 1 is needed from the full-resolution lists, so only the DEPTHS are
             // staged (4 of the 12 bytes per fragment) and the winner's colour is fetched directly
@@ -650,7 +652,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 e_d1 = own.n ? own.d1 : 1.0f;
                 e_tt = own.t_tail;
             }
-            if (kMode == NOIT_RESOLVE_ADAPTIVE && mixed && p < A.P) {
+            if (kCoarse && mixed && p < A.P) {
                 // S7 / O7g: layer 2 and / or the raw tail accumulators of this pixel come from a
                 // coarse buffer's G, bilinearly sampled at the pixel centre; layer 1 stays
                 // the full-resolution one
@@ -658,7 +660,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 const int plod = lane_lod(p, plevel);                // of the OWNED pixel
                 const int y = (int)(p / (uint32_t)A.W), x = (int)(p - (uint32_t)y * (uint32_t)A.W);
                 float G2[10], G3[10];
-                if (A.pass_scales) {                                 // frame-global lods, image clamp
+                if (kGlobal) {                                       // frame-global lods, image clamp
                     if (g_lod2 > 0)
                         sample_coarse_g(A.coarse_g[g_lod2 - 1], A.coarse_w[g_lod2 - 1], A.coarse_h[g_lod2 - 1],
                                         g_lod2, 30, x, y, G2);
@@ -755,6 +757,9 @@ noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int
     case NOIT_RESOLVE_ADAPTIVE:
         return f16 ? launch_mode<__half, NOIT_RESOLVE_ADAPTIVE>(ctx, A, st)
                    : launch_mode<float, NOIT_RESOLVE_ADAPTIVE>(ctx, A, st);
+    case NOIT_RESOLVE_GLOBAL:
+        return f16 ? launch_mode<__half, NOIT_RESOLVE_GLOBAL>(ctx, A, st)
+                   : launch_mode<float, NOIT_RESOLVE_GLOBAL>(ctx, A, st);
     default:
         return f16 ? launch_mode<__half, NOIT_RESOLVE_ALL>(ctx, A, st)
                    : launch_mode<float, NOIT_RESOLVE_ALL>(ctx, A, st);
