@@ -106,6 +106,23 @@ def test_adaptive_resolve_small(noit, cfg4_small):
         close(got0[k].cpu().numpy(), plain[k].cpu().numpy().astype(np.float64), extra=extra)
 
 
+def test_adaptive_resolve_ragged_size(noit):
+    """Width not a multiple of 8 (cells cut by the right edge), P not a multiple of 32 (last tile
+    partial, tiles wrap rows in the middle of a cell): the per-tile lod summary of the pre-pass
+    must agree with the per-pixel levels the oracle uses."""
+    sc = noit_scenes.cfg4(3, W=333, H=150, n_prims=64, mean_band=(8.0, 10.0), cap=48)
+    assert sc.full.width % 8 and sc.full.num_pixels % 32
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    mag = mlp_magnitude(w_eff, np.maximum(oracle.build_features(sc.full)["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for l2l, thr in (((2, 1, 0, 0), 6), ((2, 2, 1, 0), 6), ((1, 1, 1, 1), 6), ((2, 1, 0, 0), 10 ** 9)):
+        _, got, ref, cell = run_adaptive(noit, sc, l2l=l2l, thr=thr)
+        assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+        for k in ("trans", "final"):
+            close(got[k].cpu().numpy(), ref[k], extra=extra)
+            assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
+
+
 def test_adaptive_all_coarse(noit, cfg4_small):
     """Force every leaf coarse (huge threshold => all 64-leaves => quarter res everywhere)."""
     sc = cfg4_small
