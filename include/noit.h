@@ -156,7 +156,12 @@ noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* desc, void* str
 /* Same as noit_resolve (plain, no S7/S9) but EVERY pointer in `desc` is a HOST pointer: the
  * call stages the fragment buffer into context-owned device memory (grown on demand, kept
  * between calls), runs the fused kernel and copies the requested outputs back.  Returns after
- * the outputs are in host memory.  Pinned host memory makes the copies asynchronous DMA.     */
+ * the outputs are in host memory.  Pinned host memory makes the copies asynchronous DMA.
+ * Frames above 32 MB are pipelined in up to 8 bands of whole 32-pixel tiles: the host->device
+ * copies, the kernels (on `stream`) and the device->host copies run on three streams chained by
+ * events, so the outputs travel back while later inputs still arrive; results are bit-identical
+ * to the single launch.  The call reads host_desc->full.offsets on the host to cut the bands
+ * (NOIT_ERR_FORMAT if they are not monotone within [0, F]).                                    */
 noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* host_desc, void* stream);
 
 /* ---- S6 quadtree split (sizes 64->8 per BASELINE.json cfg4, A13; O6).

@@ -79,6 +79,10 @@ void noit_destroy(noit_ctx* ctx)
     cudaFree(ctx->d_coarse_g[0]);
     cudaFree(ctx->d_coarse_g[1]);
     cudaFree(ctx->d_stage);
+    if (ctx->h2d_stream) cudaStreamDestroy(ctx->h2d_stream);
+    if (ctx->d2h_stream) cudaStreamDestroy(ctx->d2h_stream);
+    for (cudaEvent_t e : ctx->host_ev)
+        if (e) cudaEventDestroy(e);
     cudaFree(ctx->d_tile_depth);
     delete ctx;
 }

@@ -35,6 +35,7 @@ struct MlpWeightsT {
 };
 static_assert(sizeof(MlpWeightsT) <= 4096, "fits the classic kernel-parameter space");
 
+#define NOIT_HOST_BANDS 8
 struct noit_ctx {
     int device = 0;
     bool has_weights = false;
@@ -55,6 +56,10 @@ struct noit_ctx {
     // staging for noit_resolve_host
     void* d_stage = nullptr;
     size_t stage_cap = 0;
+    // noit_resolve_host pipelines the frame in bands: H2D copies, kernels (caller's stream) and
+    // D2H copies run on three streams chained by events (created on first use)
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    cudaEvent_t host_ev[2 * NOIT_HOST_BANDS + 2] = {};
     int num_sms = 148;
 };
 

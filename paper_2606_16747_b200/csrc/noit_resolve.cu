@@ -1,6 +1,8 @@
 // noit_resolve.cu -- noit_resolve / noit_resolve_host: host-side checks and dispatch, and the S7
 // pre-pass (coarse_g_kernel).  Every resolve (plain frame, S7 adaptive, S9 pixel list) runs in
 // the staged kernel (noit_resolve_staged.cu).
+#include <algorithm>
+
 #include "noit_resolve_common.cuh"
 
 noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt, int mode,
@@ -244,25 +246,79 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* s
         ctx->stage_cap = total;
     }
     char* base = static_cast<char*>(ctx->d_stage);
-    NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_off, h->full.offsets, 4 * (P + 1), cudaMemcpyHostToDevice, st));
-    if (F) {
-        NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_depth, h->full.depth, 4 * F, cudaMemcpyHostToDevice, st));
-        NOIT_CUDA(ctx, cudaMemcpyAsync(base + o_rgba, h->full.rgba, cb * F, cudaMemcpyHostToDevice, st));
+    // Bands of whole 32-pixel tiles, pipelined over three streams: band b+1 is copied in while band
+    // b is resolved and band b-1 is copied out (the CSR lists of a pixel range are one contiguous
+    // fragment range, so a band is three contiguous H2D copies).  The link is full duplex, so the
+    // outputs travel while the inputs still arrive; the kernels (19 us per band at 1080p) hide
+    // entirely.  Small frames go in one band.
+    if (!ctx->h2d_stream) {
+        NOIT_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->h2d_stream, cudaStreamNonBlocking));
+        NOIT_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->d2h_stream, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : ctx->host_ev) NOIT_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    noit_resolve_desc d = *h;
-    d.full.offsets = reinterpret_cast<const uint32_t*>(base + o_off);
-    d.full.depth = reinterpret_cast<const float*>(base + o_depth);
-    d.full.rgba = base + o_rgba;
-    d.out_trans = h->out_trans ? reinterpret_cast<float*>(base + o_trans) : nullptr;
-    d.out_final = h->out_final ? reinterpret_cast<float*>(base + o_final) : nullptr;
-    d.out_depth1 = h->out_depth1 ? reinterpret_cast<float*>(base + o_d1) : nullptr;
-    NOIT_TRY(resolve_device(ctx, &d, st));
-    if (h->out_trans)
-        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_trans, d.out_trans, 16 * P, cudaMemcpyDeviceToHost, st));
-    if (h->out_final)
-        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_final, d.out_final, 16 * P, cudaMemcpyDeviceToHost, st));
-    if (h->out_depth1)
-        NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_depth1, d.out_depth1, 4 * P, cudaMemcpyDeviceToHost, st));
+    const uint32_t* hoff = h->full.offsets;               // HOST memory
+    const size_t in_bytes = 4 * (P + 1) + (4 + cb) * F;
+    const size_t nb = std::min<size_t>(NOIT_HOST_BANDS, std::max<size_t>(1, in_bytes >> 24));
+    const size_t band_px = (((P + nb - 1) / nb) + 31) & ~(size_t)31;
+    cudaEvent_t* ev_h2d = ctx->host_ev;
+    cudaEvent_t* ev_k = ctx->host_ev + NOIT_HOST_BANDS;
+    cudaEvent_t ev_start = ctx->host_ev[2 * NOIT_HOST_BANDS], ev_done = ctx->host_ev[2 * NOIT_HOST_BANDS + 1];
+    // the staging area is reused between calls: the copies start after the caller's earlier work
+    NOIT_CUDA(ctx, cudaEventRecord(ev_start, st));
+    NOIT_CUDA(ctx, cudaStreamWaitEvent(ctx->h2d_stream, ev_start, 0));
+    NOIT_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h_stream, ev_start, 0));
+    uint32_t* d_off = reinterpret_cast<uint32_t*>(base + o_off);
+    float* d_depth = reinterpret_cast<float*>(base + o_depth);
+    char* d_rgba = base + o_rgba;
+    float* d_trans = h->out_trans ? reinterpret_cast<float*>(base + o_trans) : nullptr;
+    float* d_final = h->out_final ? reinterpret_cast<float*>(base + o_final) : nullptr;
+    float* d_d1 = h->out_depth1 ? reinterpret_cast<float*>(base + o_d1) : nullptr;
+    size_t band = 0;
+    for (size_t p0 = 0; p0 < P; p0 += band_px, ++band) {
+        const size_t p1 = std::min(P, p0 + band_px), np = p1 - p0;
+        const size_t f0 = hoff[p0], f1 = hoff[p1];
+        if (f1 < f0 || f1 > F)
+            return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_resolve_host: offsets are not a CSR of F fragments");
+        NOIT_CUDA(ctx, cudaMemcpyAsync(d_off + p0, hoff + p0, 4 * (np + 1), cudaMemcpyHostToDevice, ctx->h2d_stream));
+        if (f1 > f0) {
+            NOIT_CUDA(ctx, cudaMemcpyAsync(d_depth + f0, h->full.depth + f0, 4 * (f1 - f0), cudaMemcpyHostToDevice,
+                                           ctx->h2d_stream));
+            NOIT_CUDA(ctx, cudaMemcpyAsync(d_rgba + cb * f0, static_cast<const char*>(h->full.rgba) + cb * f0,
+                                           cb * (f1 - f0), cudaMemcpyHostToDevice, ctx->h2d_stream));
+        }
+        NOIT_CUDA(ctx, cudaEventRecord(ev_h2d[band], ctx->h2d_stream));
+        NOIT_CUDA(ctx, cudaStreamWaitEvent(st, ev_h2d[band], 0));
+        // the band as a frame of its own: np pixels whose lists index the whole fragment arrays
+        // (a tile's copy is rounded to 4 fragments, so it may read up to 3 fragments of the
+        // neighbouring bands -- staged, never scanned)
+        ResolveArgs A;
+        memset(&A, 0, sizeof A);
+        A.W = h->full.width;
+        A.H = h->full.height;
+        A.P = (uint32_t)np;
+        A.F = (uint32_t)F;
+        A.offsets = d_off + p0;
+        A.depth = d_depth;
+        A.rgba = d_rgba;
+        memcpy(A.bg, h->background, sizeof A.bg);
+        A.out_trans = d_trans ? d_trans + 4 * p0 : nullptr;
+        A.out_final = d_final ? d_final + 4 * p0 : nullptr;
+        A.out_depth1 = d_d1 ? d_d1 + p0 : nullptr;
+        NOIT_TRY(noit_launch_resolve_staged(ctx, A, h->full.color_fmt, NOIT_RESOLVE_ALL, st));
+        NOIT_CUDA(ctx, cudaEventRecord(ev_k[band], st));
+        NOIT_CUDA(ctx, cudaStreamWaitEvent(ctx->d2h_stream, ev_k[band], 0));
+        if (h->out_trans)
+            NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_trans + 4 * p0, d_trans + 4 * p0, 16 * np, cudaMemcpyDeviceToHost,
+                                           ctx->d2h_stream));
+        if (h->out_final)
+            NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_final + 4 * p0, d_final + 4 * p0, 16 * np, cudaMemcpyDeviceToHost,
+                                           ctx->d2h_stream));
+        if (h->out_depth1)
+            NOIT_CUDA(ctx, cudaMemcpyAsync(h->out_depth1 + p0, d_d1 + p0, 4 * np, cudaMemcpyDeviceToHost,
+                                           ctx->d2h_stream));
+    }
+    NOIT_CUDA(ctx, cudaEventRecord(ev_done, ctx->d2h_stream));
+    NOIT_CUDA(ctx, cudaStreamWaitEvent(st, ev_done, 0));
     NOIT_CUDA(ctx, cudaStreamSynchronize(st));
     return NOIT_OK;
 }

@@ -296,3 +296,23 @@ def test_resolve_host_matches_device(noit, cfg1_scene):
     assert np.array_equal(trans, dev["trans"].cpu().numpy())
     assert np.array_equal(final, dev["final"].cpu().numpy())
     assert np.array_equal(d1, dev["depth1"].cpu().numpy())
+
+
+def test_resolve_host_banded_matches_device(noit, cfg2_scene, cfg3_scene):
+    """noit_resolve_host pipelines frames above 32 MB in bands of whole tiles over three streams
+    (cfg2: 5 bands, cfg3: 8): every band boundary must give the same bits as the single launch,
+    twice in a row on the same context (the staging area is reused), from pinned and from
+    pageable host memory."""
+    for sc in (cfg2_scene, cfg3_scene):
+        ctx = noit.Noit(sc.weights, sc.mlp_precision)
+        dev = ctx.resolve(noit.DeviceFragBuf.from_host(sc.full), BG)
+        P = sc.full.num_pixels
+        for pinned in (False, True, True):
+            mk = (lambda *sh: torch.zeros(sh, dtype=torch.float32).pin_memory()) if pinned else \
+                (lambda *sh: np.zeros(sh, np.float32))
+            trans, final, d1 = mk(P, 4), mk(P, 4), mk(P)
+            ctx.resolve_host(sc.full, BG, trans, final, d1)
+            for got, want in ((trans, dev["trans"]), (final, dev["final"]), (d1, dev["depth1"])):
+                got = got.numpy() if pinned else got
+                assert np.array_equal(got, want.cpu().numpy())
+
