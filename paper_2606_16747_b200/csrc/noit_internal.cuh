@@ -51,7 +51,7 @@ struct noit_ctx {
     uint32_t* d_counters = nullptr;  // small zero-initialised work counters
     float* d_coarse_g[2] = {nullptr, nullptr};   // S7: G[10] per half / quarter pixel
     size_t coarse_g_cap[2] = {0, 0};
-    uint8_t* d_tile_depth = nullptr;             // NEXT-1: per-tile subtree depth before balancing
+    uint32_t* d_tile_depth = nullptr;            // NEXT-1: balanced masks before they are published (u32 per tile)
     size_t tile_depth_cap = 0;
     // staging for noit_resolve_host
     void* d_stage = nullptr;

@@ -311,28 +311,28 @@ extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t 
 // ------------------------------------------------------------------------------------------
 // NEXT-1: quadtree consistency + demand index (O10, reading A25)
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-tile_depth_kernel(const uint32_t* __restrict__ tile_mask, int n, uint8_t* __restrict__ depth)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) depth[i] = (uint8_t)mask_depth(tile_mask[i]);
-}
-
 // One warp per base tile.  k Jacobi steps of L <- max(L, max over edge neighbours of L - 1)
 // equal the max-plus convolution of the initial depths with the Manhattan diamond of radius k
 // (induction on k), so each tile is finished in one pass over its diamond -- no ping-pong
 // buffers, no grid synchronisation.  A tile that rises to depth L is refined uniformly to L.
-// The last block to finish turns the histogram into w = sum l N_l / sum N_l and
-// s_p = clamp(2^(w - delta_p), 0.25, 1) (Eq. 2).
+// The masks are balanced "in place" for the caller, but no tile may see a neighbour's balanced
+// mask: every warp reads the ORIGINAL masks (depth of a subtree = three bit tests), writes its
+// balanced mask to a scratch array, and the last block to finish (atomic ticket) copies the
+// scratch over tile_mask -- one launch, no depth pre-pass, no grid synchronisation.  The leaf
+// histogram is accumulated in context counters (re-armed by the last block), so the caller's
+// level_hist needs no memset either.  The last block also turns the histogram into
+// w = sum l N_l / sum N_l and s_p = clamp(2^(w - delta_p), 0.25, 1) (Eq. 2).
 __global__ void __launch_bounds__(128)
-balance_kernel(const uint8_t* __restrict__ depth0, int W, int H, int Tx, int Ty, int k, float delta2,
-               float delta3, uint32_t* __restrict__ tile_mask, uint8_t* __restrict__ tile_level,
-               uint8_t* __restrict__ cell_level, uint32_t* __restrict__ hist, float* __restrict__ scales,
-               uint32_t* __restrict__ ticket)
+balance_kernel(int W, int H, int Tx, int Ty, int k, float delta2, float delta3,
+               uint32_t* __restrict__ tile_mask, uint32_t* __restrict__ mask_tmp,
+               uint8_t* __restrict__ tile_level, uint8_t* __restrict__ cell_level,
+               uint32_t* __restrict__ hist_out, float* __restrict__ scales, uint32_t* __restrict__ ticket,
+               uint32_t* __restrict__ hist_acc)
 {
     const int lane = threadIdx.x & 31;
+    const int n = Tx * Ty;
     const int tile = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (tile < Tx * Ty) {
+    if (tile < n) {
         const int tx = tile % Tx, ty = tile / Tx;
         // the diamond has 2k(k+1)+1 tiles; lanes stride over its rows
         int best = 0;
@@ -342,23 +342,22 @@ balance_kernel(const uint8_t* __restrict__ depth0, int W, int H, int Tx, int Ty,
             for (int dx = -r; dx <= r; ++dx) {
                 const int x = tx + dx;
                 if (x < 0 || x >= Tx) continue;
-                best = max(best, (int)depth0[y * Tx + x] - (abs(dx) + abs(dy)));
+                best = max(best, mask_depth(__ldcg(tile_mask + y * Tx + x)) - (abs(dx) + abs(dy)));
             }
         }
         best = __reduce_max_sync(0xffffffffu, best);
-        uint32_t mask = tile_mask[tile];
+        uint32_t mask = __ldcg(tile_mask + tile);
         if (best >= 1) mask |= 1u;                       // every node above depth `best` splits
         if (best >= 2) mask |= 0x1Eu;
         if (best >= 3) mask |= 0x1FFFE0u;
         __syncwarp();
         if (lane == 0) {
-            tile_mask[tile] = mask;
+            mask_tmp[tile] = mask;
             if (tile_level) tile_level[tile] = (uint8_t)best;
         }
-        emit_levels_and_hist<3>(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist);
+        emit_levels_and_hist<3>(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist_acc);
     }
-    if (!scales) return;
-    // last block: demand index and Eq. 2
+    // last block: publish the balanced masks, the histogram, the demand index and Eq. 2
     __shared__ bool last;
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -366,16 +365,24 @@ balance_kernel(const uint8_t* __restrict__ depth0, int W, int H, int Tx, int Ty,
         last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
     __syncthreads();
-    if (last && threadIdx.x == 0) {
-        __threadfence();
-        uint32_t n[4];
-        for (int l = 0; l < 4; ++l) n[l] = atomicAdd(hist + l, 0u);
-        const float den = (float)(n[0] + n[1] + n[2] + n[3]);
-        const float w = den > 0.f ? __fdiv_rn((float)(n[1] + 2u * n[2] + 3u * n[3]), den) : 0.f;
-        scales[0] = w;
-        scales[1] = fminf(fmaxf(exp2f(w - delta2), 0.25f), 1.0f);
-        scales[2] = fminf(fmaxf(exp2f(w - delta3), 0.25f), 1.0f);
-        *ticket = 0u;                                    // re-arm for the next call
+    if (!last) return;
+    __threadfence();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) tile_mask[i] = __ldcg(mask_tmp + i);
+    if (threadIdx.x == 0) {
+        uint32_t nl[4];
+        for (int l = 0; l < 4; ++l) {
+            nl[l] = __ldcg(hist_acc + l);
+            hist_acc[l] = 0u;                            // re-arm for the next call
+            if (hist_out) hist_out[l] = nl[l];
+        }
+        if (scales) {
+            const float den = (float)(nl[0] + nl[1] + nl[2] + nl[3]);
+            const float w = den > 0.f ? __fdiv_rn((float)(nl[1] + 2u * nl[2] + 3u * nl[3]), den) : 0.f;
+            scales[0] = w;
+            scales[1] = fminf(fmaxf(exp2f(w - delta2), 0.25f), 1.0f);
+            scales[2] = fminf(fmaxf(exp2f(w - delta3), 0.25f), 1.0f);
+        }
+        *ticket = 0u;
     }
 }
 
@@ -402,15 +409,13 @@ extern "C" noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32
             ctx->d_tile_depth = nullptr;
             ctx->tile_depth_cap = 0;
         }
-        NOIT_CUDA(ctx, cudaMalloc(&ctx->d_tile_depth, (size_t)n));
+        NOIT_CUDA(ctx, cudaMalloc(&ctx->d_tile_depth, (size_t)n * sizeof(uint32_t)));
         ctx->tile_depth_cap = (size_t)n;
     }
-    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
-    tile_depth_kernel<<<(n + 255) / 256, 256, 0, st>>>(tile_mask, n, ctx->d_tile_depth);
-    balance_kernel<<<(n + 3) / 4, 128, 0, st>>>(ctx->d_tile_depth, width, height, Tx, Ty, iterations,
-                                                delta2, delta3, tile_mask, tile_level, cell_level,
-                                                level_hist, scales, ctx->d_counters + 2);
-    ctx->launches += 2;
+    balance_kernel<<<(n + 3) / 4, 128, 0, st>>>(width, height, Tx, Ty, iterations, delta2, delta3, tile_mask,
+                                                ctx->d_tile_depth, tile_level, cell_level, level_hist, scales,
+                                                ctx->d_counters + 2, ctx->d_counters + 4);
+    ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
 }
