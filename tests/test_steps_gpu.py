@@ -576,3 +576,81 @@ def test_abi_errors(noit, cfg1_scene):
         ctx.quadtree(out, 0, 64)
     assert L.noit_infer(ctx._ctx, None, C.c_uint32(5), None, None) == 1
     assert L.noit_last_error(None) is not None
+
+
+# -------------------------------------------------------------------------------------------
+# the launch configuration bench.py times: the whole step as ONE CUDA graph with frame 3
+# (reprojection + fallback, second context, side stream) forked beside frame 2 (quadtree +
+# balance + adaptive resolve) after the plain resolve
+# -------------------------------------------------------------------------------------------
+def test_forked_graph_step_equals_the_eager_step_and_the_oracle(noit, cfg4_small):
+    sc = cfg4_small
+    W, H, P = sc.full.width, sc.full.height, sc.full.num_pixels
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    ctx, ctx_b = noit.Noit(sc.weights, sc.mlp_precision), noit.Noit(sc.weights, sc.mlp_precision)
+    M = np.eye(4, dtype=np.float32)
+    M[0, 3] = 2.0 * 1.5 / W                                                    # 1.5-pixel camera shift
+    f32 = dict(dtype=torch.float32, device="cuda")
+    plain = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
+    adapt = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
+    st = dict(qt=None, bal=None, rp=None)
+    side = torch.cuda.Stream()
+
+    def frame3(c):
+        st["rp"] = c.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"], out=st["rp"])
+        rp = st["rp"]
+        c.resolve(fb, BG, want=(), out=dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"]),
+                  pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
+
+    def frame2():
+        st["qt"] = ctx.quadtree(plain["final"], W, H, 0, 6, out=st["qt"])
+        st["bal"] = ctx.quadtree_balance(st["qt"]["tile_mask"], W, H, out=st["bal"])
+        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=st["bal"]["cell_level"])
+
+    def serial():
+        ctx.resolve(fb, BG, want=(), out=plain)
+        frame2()
+        frame3(ctx)
+
+    def forked():
+        cur = torch.cuda.current_stream()
+        ctx.resolve(fb, BG, want=(), out=plain)
+        side.wait_stream(cur)
+        with torch.cuda.stream(side):
+            frame3(ctx_b)
+        frame2()
+        cur.wait_stream(side)
+
+    serial()
+    torch.cuda.synchronize()
+    keys = lambda: (plain["final"], adapt["final"], adapt["depth1"], st["rp"]["final"], st["rp"]["trans"],
+                    st["rp"]["accept"], st["bal"]["cell_level"], st["qt"]["tile_mask"])
+    snap = [t.clone() for t in keys()]
+    n_rej = int(st["rp"]["reject_count"].item())
+    assert 0 < n_rej < P
+    forked()                                                                   # eager once: allocations
+    torch.cuda.synchronize()
+    for t in keys():                                                           # the replay must rewrite them
+        if t.dtype == torch.float32:
+            t.zero_()
+    graph = torch.cuda.CUDAGraph()
+    capture_stream = torch.cuda.Stream()
+    with torch.cuda.graph(graph, stream=capture_stream):
+        forked()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(snap, keys()):
+        assert torch.equal(a, b)
+    assert int(st["rp"]["reject_count"].item()) == n_rej
+    # and the serial eager step is the oracle's step (frame 3 = accepted + re-resolved pixels)
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    r = oracle.resolve(sc.full, w_eff, BG)
+    rp = oracle.reproject(W, H, M, 1e-3, BG, plain["trans"].cpu().numpy(), plain["depth1"].cpu().numpy(),
+                          plain["depth1"].cpu().numpy())
+    assert np.array_equal(rp["accept"], st["rp"]["accept"].cpu().numpy())
+    assert np.array_equal(r["depth1"], plain["depth1"].cpu().numpy())
+    out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+    oracle.resolve(sc.full, w_eff, BG, pixel_list=rp["reject_list"], out=out)
+    close(st["rp"]["final"].cpu().numpy(), out["final"])
+
