@@ -255,7 +255,10 @@ def run_ours(args):
     # on a side stream through a context of its own (a context's scratch -- tile counters -- is
     # stream-ordered, include/noit.h).
     ctx_b = noit.Noit(sc.weights, sc.mlp_precision)
-    side = torch.cuda.Stream(device=dev)
+    # the critical chain (frame 1 -> frame 2) is captured on a high-priority stream, frame 3 on a
+    # default-priority one: where both have CTAs pending, the critical chain's go first
+    side = torch.cuda.Stream(device=dev, priority=0)
+    main_hp = torch.cuda.Stream(device=dev, priority=-1)
 
     def step_forked():
         nonlocal qt, bal, rp
@@ -302,7 +305,7 @@ def run_ours(args):
         def time_graph(fn):
             snap = (plain["final"].clone(), adapt["final"].clone(), rp["final"].clone(), rp["trans"].clone())
             graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph):
+            with torch.cuda.graph(graph, stream=main_hp):
                 fn()
             for _ in range(3):
                 graph.replay()
