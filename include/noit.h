@@ -174,7 +174,7 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* host_desc,
  *       pixels of the Euclidean RGB distance (fp32, fixed order); split iff D > corner_threshold
  *   tile_mask [Ty*Tx]: bit 0 root; bit 1+c level-1 child c = cx+2cy; bit 5+4c+g level-2 child
  *   cell_level [ceil(H/8)*ceil(W/8)]: level 0..3 of the leaf containing the 8x8 cell
- *   level_hist [4] (zeroed by the call): leaves per level with >= 1 in-image pixel    */
+ *   level_hist [4] (overwritten by the call): leaves per level with >= 1 in-image pixel */
 typedef struct {
     int32_t metric;
     uint32_t var_threshold_q;      /* summed-over-channels variance, 8-bit units squared      */

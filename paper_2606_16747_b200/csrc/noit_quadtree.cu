@@ -125,7 +125,8 @@ __device__ __forceinline__ void emit_levels_and_hist(uint32_t mask, int X, int Y
 __global__ void __launch_bounds__(256, 4)
 quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint32_t var_thr,
                 float corner_thr, QtTemporal tq, uint32_t* __restrict__ tile_mask,
-                uint8_t* __restrict__ cell_level, uint32_t* __restrict__ hist)
+                uint8_t* __restrict__ cell_level, uint32_t* __restrict__ hist_out,
+                uint32_t* __restrict__ hist_acc, uint32_t* __restrict__ ticket)
 {
     __shared__ Moments cell[64];          // 8x8 cells, index cy*8 + cx
     __shared__ Moments node2[16];         // level-2 nodes (16x16 pixels), index 4c + g
@@ -250,7 +251,22 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
         }
     }
     if (tile_mask && lane == 0) tile_mask[tile] = mask;
-    emit_levels_and_hist<3>(mask, X, Y, W, H, lane, cell_level, hist);
+    emit_levels_and_hist<3>(mask, X, Y, W, H, lane, cell_level, hist_out ? hist_acc : nullptr);
+    // the histogram is accumulated in context counters and published by the last tile (atomic
+    // ticket), which also re-arms them: the caller's level_hist needs no memset before the launch
+    if (!hist_out) return;
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence();
+        if (atomicAdd(ticket, 1u) == gridDim.x - 1) {
+            __threadfence();
+            for (int l = 0; l < 4; ++l) {
+                hist_out[l] = __ldcg(hist_acc + l);
+                hist_acc[l] = 0u;
+            }
+            *ticket = 0u;
+        }
+    }
 }
 
 static noit_status quadtree_launch(noit_ctx* ctx, const char* who, const float* image, int32_t width,
@@ -267,10 +283,10 @@ static noit_status quadtree_launch(noit_ctx* ctx, const char* who, const float* 
     if (!noit_aligned(image, 16))
         return noit_fail(ctx, NOIT_ERR_FORMAT, "%s: image needs 16-byte alignment", who);
     cudaStream_t st = (cudaStream_t)stream;
-    if (level_hist) NOIT_CUDA(ctx, cudaMemsetAsync(level_hist, 0, 4 * sizeof(uint32_t), st));
     const int Tx = (width + 63) / 64, Ty = (height + 63) / 64;
     quadtree_kernel<<<Tx * Ty, 256, 0, st>>>(image, width, height, metric, var_thr, corner_thr, tq,
-                                             tile_mask, cell_level, level_hist);
+                                             tile_mask, cell_level, level_hist, ctx->d_counters + 8,
+                                             ctx->d_counters + 12);
     ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
