@@ -348,18 +348,20 @@ balance_kernel(int W, int H, int Tx, int Ty, int k, float delta2, float delta3,
     const int lane = threadIdx.x & 31;
     const int n = Tx * Ty;
     const int tile = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    __shared__ uint32_t block_hist[4];                   // one set of global atomics per block
+    if (threadIdx.x < 4) block_hist[threadIdx.x] = 0u;
+    __syncthreads();
     if (tile < n) {
         const int tx = tile % Tx, ty = tile / Tx;
-        // the diamond has 2k(k+1)+1 tiles; lanes stride over its rows
+        // the diamond has 2k(k+1)+1 tiles; lanes stride over its bounding square, one independent
+        // load per lane and step (k = 2: 13 of 25 cells, a single step)
         int best = 0;
-        for (int dy = -k + lane; dy <= k; dy += 32) {
-            const int y = ty + dy, r = k - abs(dy);
-            if (y < 0 || y >= Ty) continue;
-            for (int dx = -r; dx <= r; ++dx) {
-                const int x = tx + dx;
-                if (x < 0 || x >= Tx) continue;
-                best = max(best, mask_depth(__ldcg(tile_mask + y * Tx + x)) - (abs(dx) + abs(dy)));
-            }
+        const int side = 2 * k + 1;
+        for (int i = lane; i < side * side; i += 32) {
+            const int dy = i / side - k, dx = i - (dy + k) * side - k;
+            const int dist = abs(dx) + abs(dy), x = tx + dx, y = ty + dy;
+            if (dist > k || x < 0 || x >= Tx || y < 0 || y >= Ty) continue;
+            best = max(best, mask_depth(__ldcg(tile_mask + y * Tx + x)) - dist);
         }
         best = __reduce_max_sync(0xffffffffu, best);
         uint32_t mask = __ldcg(tile_mask + tile);
@@ -371,12 +373,14 @@ balance_kernel(int W, int H, int Tx, int Ty, int k, float delta2, float delta3,
             mask_tmp[tile] = mask;
             if (tile_level) tile_level[tile] = (uint8_t)best;
         }
-        emit_levels_and_hist<3>(mask, tx << 6, ty << 6, W, H, lane, cell_level, hist_acc);
+        emit_levels_and_hist<3>(mask, tx << 6, ty << 6, W, H, lane, cell_level, block_hist);
     }
     // last block: publish the balanced masks, the histogram, the demand index and Eq. 2
     __shared__ bool last;
     __syncthreads();
     if (threadIdx.x == 0) {
+        for (int l = 0; l < 4; ++l)
+            if (block_hist[l]) atomicAdd(hist_acc + l, block_hist[l]);
         __threadfence();
         last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
