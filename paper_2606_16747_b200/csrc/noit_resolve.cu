@@ -22,8 +22,9 @@ struct CoarseLevel {
     const void* rgba;
     float* G;
 };
+constexpr int kPreBlock = 256;     // threads per block of the pre-pass
 template <typename ColorT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kPreBlock)
 coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, uint32_t blocks12, int full_w,
                 const uint8_t* __restrict__ cell_level, uchar4 level_to_lod, uint8_t* __restrict__ tile_lod,
                 uint32_t num_tiles, uint32_t P)
@@ -175,7 +176,7 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
             A.coarse_h[lod - 1] = cb->height;
             lv[lod - 1] = CoarseLevel{cb->width, cb->height, cb->offsets, cb->depth, cb->rgba,
                                       ctx->d_coarse_g[lod - 1]};
-            blocks[lod - 1] = (uint32_t)((cp + 127) / 128);
+            blocks[lod - 1] = (uint32_t)((cp + kPreBlock - 1) / kPreBlock);
         }
         // per-tile mode with no level mapped to a coarse lod: the frame is a plain resolve
         if (d->cell_level && blocks[0] + blocks[1] == 0)
@@ -194,15 +195,15 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
                 ctx->tile_lod_cap = num_tiles;
             }
             A.tile_lod = ctx->d_tile_lod;
-            blocks_s = (num_tiles + 127u) / 128u;
+            blocks_s = (num_tiles + kPreBlock - 1u) / kPreBlock;
         }
         if (blocks[0] + blocks[1] + blocks_s) {
             const uint32_t b12 = blocks[0] + blocks[1];
             if (fmt == NOIT_RGBA_F16)
-                coarse_g_kernel<__half><<<b12 + blocks_s, 128, 0, st>>>(
+                coarse_g_kernel<__half><<<b12 + blocks_s, kPreBlock, 0, st>>>(
                     lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
             else
-                coarse_g_kernel<float><<<b12 + blocks_s, 128, 0, st>>>(
+                coarse_g_kernel<float><<<b12 + blocks_s, kPreBlock, 0, st>>>(
                     lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
