@@ -96,6 +96,32 @@ template <> struct Color<__half> {
         v.y &= 0x0000FFFFu;
         return v;
     }
+    // O2's tail sums for one fragment.  sm_100a has mixed-precision fp32 += fp16 * fp16
+    // (`fma.rn.f32.f16`, SASS FHFMA, with half-select operands) and fp32 += fp16 (FHADD): the
+    // product of two halves is exact in fp32 and the sum is rounded once, i.e. bit for bit what
+    // fmaf(float(a), float(c), acc) gives -- without the three conversions (6 instead of 9
+    // instructions per fragment; only alpha is converted, for the transmittance product).
+    static __device__ __forceinline__ float fhfma(unsigned short a, unsigned short b, float c)
+    {
+        asm("fma.rn.f32.f16 %0, %1, %2, %0;" : "+f"(c) : "h"(a), "h"(b));
+        return c;
+    }
+    static __device__ __forceinline__ float fhadd(unsigned short a, float c)
+    {
+        asm("add.rn.f32.f16 %0, %1, %0;" : "+f"(c) : "h"(a));
+        return c;
+    }
+    static __device__ __forceinline__ void accumulate(Packed v, float& r, float& g, float& b, float& a, float& t)
+    {
+        const unsigned short x = (unsigned short)(v.x & 0xffffu), y = (unsigned short)(v.x >> 16);
+        const unsigned short z = (unsigned short)(v.y & 0xffffu), w = (unsigned short)(v.y >> 16);
+        r = fhfma(w, x, r);
+        g = fhfma(w, y, g);
+        b = fhfma(w, z, b);
+        a = fhadd(w, a);
+        const float wf = __half2float(__ushort_as_half(w));
+        t = fmaf(-wf, t, t);                               // t *= (1 - alpha), one rounding
+    }
 };
 template <> struct Color<float> {
     typedef float4 Packed;
@@ -104,6 +130,14 @@ template <> struct Color<float> {
     static __device__ __forceinline__ float4 unpack(Packed v) { return v; }
     static __device__ __forceinline__ void zero_alpha(Packed* slot) { slot->w = 0.f; }
     static __device__ __forceinline__ Packed zero_alpha_reg(Packed v) { v.w = 0.f; return v; }
+    static __device__ __forceinline__ void accumulate(Packed c, float& r, float& g, float& b, float& a, float& t)
+    {
+        r = fmaf(c.w, c.x, r);
+        g = fmaf(c.w, c.y, g);
+        b = fmaf(c.w, c.z, b);
+        a += c.w;
+        t = fmaf(-c.w, t, t);                              // t *= (1 - alpha), one rounding
+    }
 };
 
 // key (depth, index) lexicographic (O1)
@@ -178,14 +212,7 @@ __device__ __forceinline__ Sums scan_colours(const typename Color<ColorT>::Packe
     Sums s;
     s.r = s.g = s.b = s.a = 0.f;
     s.t = 1.f;
-    auto acc = [&](Packed raw) {
-        const float4 c = Color<ColorT>::unpack(raw);
-        s.r = fmaf(c.w, c.x, s.r);
-        s.g = fmaf(c.w, c.y, s.g);
-        s.b = fmaf(c.w, c.z, s.b);
-        s.a += c.w;
-        s.t = fmaf(-c.w, s.t, s.t);                    // t *= (1 - alpha), one rounding
-    };
+    auto acc = [&](Packed raw) { Color<ColorT>::accumulate(raw, s.r, s.g, s.b, s.a, s.t); };
     uint32_t pos = first;
 #pragma unroll 1
     for (; pos + S < end; pos += 2 * S) {
@@ -273,10 +300,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
         for (uint32_t j = b + q; j < e; j += L) {
             typename Color<ColorT>::Packed raw = __ldg(rgba + j);
             if (j == s.i1 || j == s.i2) raw = Color<ColorT>::zero_alpha_reg(raw);
-            const float4 c = Color<ColorT>::unpack(raw);
-            ar = fmaf(c.w, c.x, ar); ag = fmaf(c.w, c.y, ag); ab = fmaf(c.w, c.z, ab);
-            at += c.w;
-            tt = fmaf(-c.w, tt, tt);
+            Color<ColorT>::accumulate(raw, ar, ag, ab, at, tt);
         }
 #pragma unroll
         for (int m = 1; m < L; m <<= 1) {
