@@ -590,6 +590,145 @@ def test_reproject_depth_threshold_and_w_sign():
     assert not oracle.reproject(W, H, M, tau, BG, trans, prev, cur)["accept"].any()
 
 
+# ---- O8: the homogeneous divide, the depth row, the whole transform chain --------------------
+# (with M = I or an NDC translation c_3 is always 1 and row 2 of M is always
+#  (0,0,1,0), so a dropped "/ c_3", "d" used for "d_e", or an ignored M[2][*] passed every pin.)
+def _index_image(W, H):
+    """prev_trans whose pixel q carries (qx, qy, q, 1): reads back which pixel was fetched."""
+    yy, xx = np.mgrid[0:H, 0:W]
+    return np.stack([xx, yy, yy * W + xx, np.ones_like(xx)], axis=-1).reshape(-1, 4).astype(np.float32)
+
+
+@pytest.mark.parametrize("s", [2.0, 0.5, 8.0])
+def test_reproject_uniform_homogeneous_scale_is_the_identity(s):
+    """M = s*I maps (x, y, d, 1) to s*(x, y, d, 1): after the divide by c_3 = s the map is the
+    identity.  s is a power of two, so every product and quotient is exact: bit for bit."""
+    rng = np.random.default_rng(40)
+    for (W, H) in ((64, 32), (317, 203)):
+        trans, depth = random_frame(rng, W, H)
+        r = oracle.reproject(W, H, s * np.eye(4), 1e-3, BG, trans, depth, depth)
+        r0 = oracle.reproject(W, H, np.eye(4), 1e-3, BG, trans, depth, depth)
+        assert r["accept"].all() and r["reject_count"] == 0
+        assert np.array_equal(r["trans"], trans) and np.array_equal(r["depth"], depth)
+        assert np.array_equal(r["final"], r0["final"])
+
+
+def test_reproject_depth_row_and_expected_depth():
+    """M = diag(1, 1, a, 1) with M[2][3] = b and M[2][0], M[2][1] = gx, gy (all dyadic, depths on a
+    2^-10 grid, W and H powers of two so x_ndc, y_ndc are dyadic): d_e = gx*xn + gy*yn + a*d + b is
+    exact in fp32, so out_depth must equal the float64 value bit for bit, and the accept test must
+    flip exactly at |prev_depth - d_e| = tau -- on d_e, not on d."""
+    W, H = 64, 32
+    rng = np.random.default_rng(41)
+    trans = _index_image(W, H)
+    d = (rng.integers(64, 960, W * H) / 1024.0).astype(np.float32)
+    yy, xx = np.mgrid[0:H, 0:W]
+    xn = (2.0 * (xx + 0.5) / W - 1.0).reshape(-1)
+    yn = (2.0 * (yy + 0.5) / H - 1.0).reshape(-1)
+    for (a, b, gx, gy) in ((0.5, 0.25, 0.0, 0.0), (0.25, 0.5, 0.125, 0.0), (0.5, 0.125, -0.0625, 0.03125)):
+        M = np.eye(4)
+        M[2, 2], M[2, 3], M[2, 0], M[2, 1] = a, b, gx, gy
+        d_e = gx * xn + gy * yn + a * d.astype(np.float64) + b           # exact in float64
+        assert np.array_equal(d_e.astype(np.float32).astype(np.float64), d_e)   # ... and in fp32
+        tau = 2.0 ** -7
+        off = np.where(rng.random(W * H) < 0.5, tau, 2.0 * tau) * np.where(rng.random(W * H) < 0.5, 1.0, -1.0)
+        prev = (d_e + off).astype(np.float32)                            # exact: dyadic sums
+        r = oracle.reproject(W, H, M, tau, BG, trans, prev, d)
+        want = np.abs(off) <= tau                                        # |prev - d_e| = tau accepts (<=)
+        assert np.array_equal(r["accept"].astype(bool), want)
+        assert np.array_equal(r["depth"][want], d_e.astype(np.float32)[want])
+        # x, y untouched by the depth row: every accepted pixel fetched itself
+        assert np.array_equal(r["trans"][want], trans[want])
+        # the test is against d_e, not against the current depth d: with prev = d nothing passes
+        # when |d - d_e| > tau everywhere
+        far = np.abs(d.astype(np.float64) - d_e) > tau
+        r2 = oracle.reproject(W, H, M, tau, BG, trans, d, d)
+        assert not r2["accept"][far].any() and far.mean() > 0.5
+
+
+def test_reproject_two_cameras_against_float64_unprojection():
+    """The whole chain against an independent float64 statement: un-project every current pixel
+    centre (with its depth) to WORLD space with inv(VP_cur), project the world point with VP_prev,
+    and read off the previous pixel and the expected depth.  The oracle gets only
+    M = VP_prev . inv(VP_cur) in fp32.  Pins row/column order of M, the pixel-centre and y-down
+    conventions (A23), the divide by c_3 on x, y AND depth, and that d_e (not d) is written."""
+    W, H = 160, 96
+    proj = noit_scenes.perspective(60.0, W / H, 0.1, 100.0)
+    vp_prev = proj @ noit_scenes.view_matrix(np.zeros(3), 0.0, 0.0)
+    vp_cur = proj @ noit_scenes.view_matrix(np.array([0.35, -0.2, 0.5]), 0.06, -0.04)
+    rng = np.random.default_rng(42)
+    # depths of points 3..30 units in front of the current camera (z_ndc = far/(far-near)*(1 - near/z))
+    z = rng.uniform(3.0, 30.0, W * H)
+    d32 = (100.0 / 99.9 * (1.0 - 0.1 / z)).astype(np.float32)
+    yy, xx = np.mgrid[0:H, 0:W]
+    xn = 2.0 * (xx.reshape(-1) + 0.5) / W - 1.0
+    yn = 2.0 * (yy.reshape(-1) + 0.5) / H - 1.0
+    ndc = np.stack([xn, yn, d32.astype(np.float64), np.ones(W * H)], axis=1)
+    world = ndc @ np.linalg.inv(vp_cur).T
+    world /= world[:, 3:4]                                   # a point in world space
+    clip = world @ vp_prev.T
+    u = (clip[:, 0] / clip[:, 3] + 1.0) * 0.5 * W
+    v = (clip[:, 1] / clip[:, 3] + 1.0) * 0.5 * H
+    d_e = clip[:, 2] / clip[:, 3]
+    M = (vp_prev @ np.linalg.inv(vp_cur)).astype(np.float32)
+    trans = _index_image(W, H)
+    prev_depth = np.zeros(W * H, np.float32)
+    r = oracle.reproject(W, H, M, 10.0, BG, trans, prev_depth, d32)     # tau = 10: only geometry rejects
+    on = (clip[:, 3] > 0) & (u >= 0) & (u < W) & (v >= 0) & (v < H)
+    edge = np.minimum(np.abs(u - np.round(u)), np.abs(v - np.round(v)))
+    safe = edge > 1e-3                                       # fp32 vs float64 may differ at a pixel edge
+    assert 0.5 < (on & safe).mean() < 1.0                    # the motion really moves pixels off screen
+    assert np.array_equal(r["accept"][safe].astype(bool), on[safe])
+    sel = on & safe
+    assert np.array_equal(r["trans"][sel, 0], np.floor(u[sel]).astype(np.float32))
+    assert np.array_equal(r["trans"][sel, 1], np.floor(v[sel]).astype(np.float32))
+    assert (np.floor(u[sel]) != xx.reshape(-1)[sel]).mean() > 0.5        # a real displacement
+    assert np.abs(r["depth"][sel].astype(np.float64) - d_e[sel]).max() <= 1e-6
+    assert np.abs(d_e[sel] - d32[sel]).max() > 1e-3          # d_e differs from d: writing d would fail
+    # the bilinear variant shares the transform, q and out_depth
+    rb = oracle.reproject_bilinear(W, H, M, 10.0, BG, trans, prev_depth, d32)
+    assert np.array_equal(rb["accept"], r["accept"]) and np.array_equal(rb["depth"], r["depth"])
+
+
+def test_quadtree_quantiser_clamps_out_of_range_colours():
+    """q = rint(255 * clamp(c, 0, 1)) (O6): the resolve's ReLU output is unbounded above (A11) and
+    is what S6 consumes.  (i) out-of-range values behave exactly like their clamped values;
+    (ii) closed forms that only a clamp produces."""
+    rng = np.random.default_rng(43)
+    W, H = 200, 136
+    img = rng.uniform(0.2, 0.8, (W * H, 4)).astype(np.float32)
+    pick = rng.random((W * H, 3))
+    vals = np.array([-0.5, 1.7, 3.0, -1e30, 1e30], np.float32)
+    for k in range(3):
+        m = pick[:, k] < 0.3
+        img[m, k] = vals[rng.integers(0, len(vals), int(m.sum()))]
+    clamped = img.copy()
+    clamped[:, :3] = np.clip(img[:, :3], 0.0, 1.0)
+    for metric, thr in ((0, 6), (0, 2000), (1, 0.02)):
+        a = oracle.quadtree(img, W, H, metric, thr if metric == 0 else 6, thr if metric == 1 else 0.02)
+        b = oracle.quadtree(clamped, W, H, metric, thr if metric == 0 else 6, thr if metric == 1 else 0.02)
+        if metric == 0:                                      # the corner metric does not quantise
+            assert np.array_equal(a["tile_mask"], b["tile_mask"])
+            assert np.array_equal(a["cell_level"], b["cell_level"]) and np.array_equal(a["hist"], b["hist"])
+    # (ii) every value >= 1 is the same colour after the clamp: a constant image, no split at all
+    hot = np.full((64 * 64, 4), 1.7, np.float32)
+    hot[rng.integers(0, 64 * 64, 200), :3] = 3.0
+    q = oracle.quadtree(hot, 64, 64, 0, 0)
+    assert q["tile_mask"][0] == 0 and q["hist"].tolist() == [1, 0, 0, 0]
+    # ... and every value <= 0 likewise
+    cold = np.full((64 * 64, 4), -0.5, np.float32)
+    cold[rng.integers(0, 64 * 64, 200), :3] = 0.0
+    assert oracle.quadtree(cold, 64, 64, 0, 0)["tile_mask"][0] == 0
+    # half of the tile at -0.5 (-> 0), half at 3.0 (-> 255): variance per channel (255/2)^2 at the
+    # root, zero inside each half: root and nothing else splits ... the halves are x < 32 / x >= 32,
+    # so the four level-1 children are constant
+    two = np.full((64, 64, 4), -0.5, np.float32)
+    two[:, 32:, :3] = 3.0
+    q2 = oracle.quadtree(two.reshape(-1, 4), 64, 64, 0, 3 * 16256 - 1)   # 3*(127.5^2) = 48768.75 > thr
+    assert q2["tile_mask"][0] == 1
+    assert oracle.quadtree(two.reshape(-1, 4), 64, 64, 0, 48769)["tile_mask"][0] == 0
+
+
 # ---- O8b (NEXT-4, A28): bilinear-filtered reprojection ---------------------------------------
 def _shift_matrix(W, H, sx, sy):
     M = np.eye(4)
