@@ -82,8 +82,8 @@ def lib():
     """Load libnoit.so (building it first if nvcc is here and the sources are newer)."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if not os.path.exists(path) or os.environ.get("NOIT_REBUILD"):
+        path = os.environ.get("NOIT_LIBRARY") or _build.LIB      # NOIT_LIBRARY: another build of libnoit
+        if path == _build.LIB and (not os.path.exists(path) or os.environ.get("NOIT_REBUILD")):
             path = _build.build()
         L = C.CDLL(path)
         L.noit_last_error.restype = C.c_char_p

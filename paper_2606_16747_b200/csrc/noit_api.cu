@@ -58,8 +58,8 @@ noit_status noit_create(noit_ctx** out)
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
         c->num_sms = sms;
-    e = cudaMalloc(&c->d_counters, 64 * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, 64 * sizeof(uint32_t));
+    e = cudaMalloc(&c->d_counters, NOIT_COUNTER_WORDS * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, NOIT_COUNTER_WORDS * sizeof(uint32_t));
     if (e != cudaSuccess) {
         noit_cuda_check(nullptr, e, "noit_create scratch");
         delete c;

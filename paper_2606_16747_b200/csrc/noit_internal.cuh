@@ -36,6 +36,10 @@ struct MlpWeightsT {
 static_assert(sizeof(MlpWeightsT) <= 4096, "fits the classic kernel-parameter space");
 
 #define NOIT_HOST_BANDS 8
+// work counters: [0, 64) small counters of the quadtree / balance / resolve kernels, then the
+// resolve's ticket counters, one per 128-byte line
+#define NOIT_TICKET_COUNTERS_LOG2 2
+#define NOIT_COUNTER_WORDS (64 + 32 * (1 << NOIT_TICKET_COUNTERS_LOG2))
 struct noit_ctx {
     int device = 0;
     bool has_weights = false;
@@ -263,14 +267,30 @@ __device__ __forceinline__ void c_to_a(const float (&c)[4], float (&hi)[4], floa
 // All 32 lanes must call this.  x = this lane's features; scratch = 32 x 12 floats of shared
 // memory private to the warp; f = tail colour of this lane's pixel; wv = this lane's packed
 // weights, wv[v] = wp[v*32 + lane].
-__device__ __forceinline__ void mlp_forward_mma(const float4 (&wv)[NOIT_MMA_CHUNKS], float* scratch,
+// Weight sources: registers (the 10 float4 of this lane, loaded once per tile) or the CTA's copy
+// of the packed block in shared memory (read at the point of use: 40 registers fewer).
+struct MmaWeightsReg {
+    const float4 (&wv)[NOIT_MMA_CHUNKS];
+    __device__ __forceinline__ float2 pair(int i) const      // packed values (i, i+1), i even
+    {
+        const float4& v = wv[i >> 2];
+        return (i & 2) ? make_float2(v.z, v.w) : make_float2(v.x, v.y);
+    }
+    __device__ __forceinline__ float4 quad(int v) const { return wv[v]; }
+};
+struct MmaWeightsSmem {
+    const float4* wl;                                        // &wsm[lane]; chunk v at wl[v * 32]
+    __device__ __forceinline__ float2 pair(int i) const
+    {
+        return *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(wl + (i >> 2) * 32) + (i & 2));
+    }
+    __device__ __forceinline__ float4 quad(int v) const { return wl[v * 32]; }
+};
+template <typename WSrc>
+__device__ __forceinline__ void mlp_forward_mma(const WSrc wsrc, float* scratch,
                                                 int lane, const float x[5], float f[3])
 {
     const int g = lane >> 2, t = lane & 3;
-    auto wf = [&](int i) -> float {                           // packed value i (constant index)
-        const float4& v = wv[i >> 2];
-        return (i & 3) == 0 ? v.x : ((i & 3) == 1 ? v.y : ((i & 3) == 2 ? v.z : v.w));
-    };
     // features -> A fragments of layer 1 through the scratch (row = lane, stride 12: no conflicts)
     __syncwarp();
     *reinterpret_cast<float4*>(scratch + 12 * lane) = make_float4(x[0], x[1], x[2], x[3]);
@@ -292,33 +312,37 @@ __device__ __forceinline__ void mlp_forward_mma(const float4 (&wv)[NOIT_MMA_CHUN
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             float c[4];
-            mma_tf32(c, ahi, wf(2 * j), wf(2 * j + 1), zero);
-            mma_tf32(c, alo, wf(2 * j), wf(2 * j + 1), c);
+            const float2 b = wsrc.pair(2 * j);
+            mma_tf32(c, ahi, b.x, b.y, zero);
+            mma_tf32(c, alo, b.x, b.y, c);
             c_to_a(c, h1hi[j], h1lo[j]);
         }
         // layer 2: 2 n-tiles, 4 k-steps (k-step s = layer-1 n-tile s)
         float h2hi[2][4], h2lo[2][4];
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-            const float bias[4] = {wv[6 + j].x, wv[6 + j].y, wv[6 + j].z, wv[6 + j].w};
+            const float4 bq = wsrc.quad(6 + j);
+            const float bias[4] = {bq.x, bq.y, bq.z, bq.w};
             float c[4];
 #pragma unroll
             for (int s = 0; s < 4; ++s) {
-                const float b0 = wf(8 + 2 * (4 * j + s)), b1 = wf(8 + 2 * (4 * j + s) + 1);
-                if (s == 0) mma_tf32(c, h1hi[s], b0, b1, bias);
-                else mma_tf32(c, h1hi[s], b0, b1, c);
-                mma_tf32(c, h1lo[s], b0, b1, c);
+                const float2 b = wsrc.pair(8 + 2 * (4 * j + s));
+                if (s == 0) mma_tf32(c, h1hi[s], b.x, b.y, bias);
+                else mma_tf32(c, h1hi[s], b.x, b.y, c);
+                mma_tf32(c, h1lo[s], b.x, b.y, c);
             }
             c_to_a(c, h2hi[j], h2lo[j]);
         }
         // layer 3: 1 n-tile (3 outputs, padded to 8), 2 k-steps
-        const float bias3[4] = {wv[9].x, wv[9].y, wv[9].z, wv[9].w};
+        const float4 b3q = wsrc.quad(9);
+        const float bias3[4] = {b3q.x, b3q.y, b3q.z, b3q.w};
         float c[4];
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
-            if (s == 0) mma_tf32(c, h2hi[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), bias3);
-            else mma_tf32(c, h2hi[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), c);
-            mma_tf32(c, h2lo[s], wf(32 + 2 * s), wf(32 + 2 * s + 1), c);
+            const float2 b = wsrc.pair(32 + 2 * s);
+            if (s == 0) mma_tf32(c, h2hi[s], b.x, b.y, bias3);
+            else mma_tf32(c, h2hi[s], b.x, b.y, c);
+            mma_tf32(c, h2lo[s], b.x, b.y, c);
         }
 #pragma unroll
         for (int k = 0; k < 4; ++k) fout[mt][k] = fmaxf(c[k], 0.f);

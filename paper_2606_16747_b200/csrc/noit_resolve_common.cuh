@@ -27,7 +27,8 @@ struct ResolveArgs {
     // staged kernel
     const float4* mlp_packed;      // per-lane MMA fragments of the weights (NOIT_MLP_BF16)
     uint32_t num_tiles;
-    uint32_t* tile_counter;        // [0] next tile, [1] finished warps; self-resetting
+    // [1] finished warps; [64 + 32 c] ticket counter c < 2^NOIT_TICKET_COUNTERS_LOG2; self-resetting
+    uint32_t* tile_counter;
 };
 
 // ADAPTIVE = per-tile lods from cell_level (S7); GLOBAL = frame-global lods from pass_scales (O7g):

@@ -36,9 +36,24 @@
 
 namespace {
 
-constexpr uint32_t kCap = 1000;          // fragments per warp stage (12000 B with fp16 colour: 16 warps/SM)
+#ifndef NOIT_X_STAGE
+#define NOIT_X_STAGE 12000
+#endif
+#ifndef NOIT_X_WARPS
+#define NOIT_X_WARPS 4
+#endif
+#ifndef NOIT_X_CTAS
+#define NOIT_X_CTAS 4
+#endif
+#ifndef NOIT_X_WSMEM
+#define NOIT_X_WSMEM 0
+#endif
+constexpr uint32_t kStageBytesFrame = NOIT_X_STAGE;   // per warp stage (1000 fragments with fp16 colour)
 constexpr uint32_t kScratchFloats = 32 * 12;   // per warp: feature / output transpose of the MMA MLP
-constexpr int kWarpsPerCta = 4;
+constexpr int kWarpsPerCta = NOIT_X_WARPS;
+constexpr bool kWeightsInSmem = NOIT_X_WSMEM != 0;
+constexpr uint32_t kWeightBytes = kWeightsInSmem ? NOIT_MMA_CHUNKS * 32 * 16 : 0;
+constexpr uint32_t kCounterShift = NOIT_TICKET_COUNTERS_LOG2;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
 {
@@ -323,13 +338,15 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
 // the kernel
 // ------------------------------------------------------------------------------------------
 template <typename ColorT, int L, bool kMma, int kMode>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, kMode == NOIT_RESOLVE_LIST ? 1 : NOIT_X_CTAS)
 resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
 {
     typedef typename Color<ColorT>::Packed Packed;
     constexpr uint32_t CB = Color<ColorT>::kBytes;
     // per warp; S9 reads global memory directly and allocates no stage (more CTAs per SM)
-    constexpr uint32_t kStageBytes = kMode == NOIT_RESOLVE_LIST ? 0u : kCap * (4u + CB);
+    // fragments of a light tile (depths and colours staged together)
+    constexpr uint32_t kCap = (kStageBytesFrame / (4u + CB)) & ~3u;
+    constexpr uint32_t kStageBytes = kMode == NOIT_RESOLVE_LIST ? 0u : kStageBytesFrame;
     // fragments when the stage holds depths only / colours only; multiples of 4 because a copy
     // is rounded up to 4 fragments
     constexpr uint32_t kCapD = (kStageBytes / 4u) & ~3u;
@@ -354,6 +371,14 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncwarp();
+    // the CTA's copy of the packed MMA weights (read at the point of use instead of held in 40 registers)
+    const float4* const wsm = reinterpret_cast<const float4*>(
+        smem_raw + kWarpsPerCta * kStageBytes + kWarpsPerCta * kScratchFloats * sizeof(float) + kWarpsPerCta * 8u);
+    if (kMma && kWeightsInSmem) {
+        for (uint32_t i = threadIdx.x; i < NOIT_MMA_CHUNKS * 32u; i += kWarpsPerCta * 32u)
+            const_cast<float4*>(wsm)[i] = __ldg(A.mlp_packed + i);
+        __syncthreads();
+    }
     uint32_t parity = 0;
 
     const uint32_t* __restrict__ offsets = A.offsets;
@@ -370,6 +395,15 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // whole round trip -- even for inline PTX under `if (lane == 0)`.  The addend below is
     // laneid + 1 under the predicate laneid == 0: not uniform to ptxas, so the atomic stays a
     // plain predicated ATOMG and nothing waits for it until the broadcast a tile later.)
+    // Tickets are dealt from 2^kCounterShift counters on separate 128-byte lines: warp w draws
+    // from counter c = w mod 2^kCounterShift, whose k-th value stands for ticket
+    // (k << kCounterShift) | c, so every counter covers an evenly interleaved share of the frame.
+    // (With ONE counter a 4K frame of short lists -- 259 200 same-address atomics -- was measured
+    // in two states, 344 us and 640 us per frame, same bytes and instructions, the second with
+    // the long-scoreboard stall 16x higher: the atomics serialise in their L2 slice.  Four
+    // counters never showed the slow state; profiles/r02_resolve.md.)
+    const uint32_t my_c = warp_id & ((1u << kCounterShift) - 1u);
+    uint32_t* const my_counter = A.tile_counter + 64u + 32u * my_c;
     auto fetch_raw = [&]() -> uint32_t {
         uint32_t t = 0;
         asm volatile("{\n"
@@ -381,9 +415,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                      "@p atom.global.add.u32 %0, [%1], inc;\n"
                      "}\n"
                      : "+r"(t)
-                     : "l"(A.tile_counter)
+                     : "l"(my_counter)
                      : "memory");
-        return lane == 0 ? t + 3u * n_warps : 0u;
+        return t;                                        // raw: turned into a ticket a tile later
     };
     // S9 (kMode LIST): "tile" t = entries [t*32/L, (t+1)*32/L) of the pixel list; the lists of a
     // tile are not contiguous, so such tiles always take the global path.
@@ -512,6 +546,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     // tiles cluster and the load imbalance costs more than the atomics)
     uint32_t t_cur = warp_id;
     uint32_t raw_nxt = warp_id + n_warps, raw_nn = warp_id + 2u * n_warps;   // then two atomics in flight
+    uint32_t n_static = 2;                               // queued values that are tickets already
     uint32_t o0 = 0, o1 = 0, pix = 0;
     bool mixed = false;                                  // S7 / O7g: some pixel of the tile has lod > 0
     bool depth_only = false;                             // ... every pixel takes layer 2 AND tail coarse
@@ -524,7 +559,11 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         first_fill(o0, o1, depth_only);
     }
     while (t_cur < num_tiles) {
-        const uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
+        uint32_t t_nxt = __shfl_sync(0xffffffffu, raw_nxt, 0);
+        // (the counter value becomes a ticket only here, behind the broadcast: nothing may depend
+        // on the atomic's result in the tile that issued it)
+        if (n_static) --n_static;
+        else t_nxt = ((t_nxt << kCounterShift) | my_c) + 3u * n_warps;
         raw_nxt = raw_nn;
         raw_nn = fetch_raw();
         uint32_t no0 = 0, no1 = 0, npix = 0;
@@ -653,7 +692,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         // the MLP's packed weights (L1-resident) are requested before the fill is issued, so they
         // are in registers when the MLP starts
         float4 wv[NOIT_MMA_CHUNKS];
-        if (kMma) {
+        if (kMma && !kWeightsInSmem) {
 #pragma unroll
             for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(A.mlp_packed + v * 32 + lane);
         }
@@ -705,7 +744,10 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                     e_tt = G2[8];
                 }
             }
-            if (kMma) mlp_forward_mma(wv, scratch, lane, xf, f);     // all 32 lanes
+            if (kMma) {                                              // all 32 lanes
+                if (kWeightsInSmem) mlp_forward_mma(MmaWeightsSmem{wsm + lane}, scratch, lane, xf, f);
+                else mlp_forward_mma(MmaWeightsReg{wv}, scratch, lane, xf, f);
+            }
             else mlp_forward_packed(W, xf, f);
             if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
@@ -713,22 +755,25 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         t_cur = t_nxt; o0 = no0; o1 = no1;
     }
     // the last warp to finish re-arms the counters for the next launch
+    // (the fence orders this warp's outstanding, result-unused ticket atomics before its finish
+    // ticket, so no late add can land after the reset)
+    uint32_t last = 0;
     if (lane == 0) {
-        const uint32_t total = gridDim.x * kWarpsPerCta;
-        if (atomicAdd(A.tile_counter + 1, 1u) == total - 1u) {
-            A.tile_counter[0] = 0u;
-            A.tile_counter[1] = 0u;
-            __threadfence();
-        }
+        __threadfence();
+        last = atomicAdd(A.tile_counter + 1, 1u) == gridDim.x * kWarpsPerCta - 1u ? 1u : 0u;
+    }
+    if (__shfl_sync(0xffffffffu, last, 0)) {
+        for (uint32_t c = lane; c < (1u << kCounterShift); c += 32u) A.tile_counter[64u + 32u * c] = 0u;
+        if (lane == 0) A.tile_counter[1] = 0u;
     }
 }
 
 template <typename ColorT, int L, bool kMma, int kMode>
 static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
 {
-    const size_t stage = kMode == NOIT_RESOLVE_LIST ? 0 : (size_t)kCap * (4u + Color<ColorT>::kBytes);
+    const size_t stage = kMode == NOIT_RESOLVE_LIST ? 0 : (size_t)kStageBytesFrame;
     const size_t smem = kWarpsPerCta * stage + kWarpsPerCta * sizeof(uint64_t) +
-                        kWarpsPerCta * kScratchFloats * sizeof(float);
+                        kWarpsPerCta * kScratchFloats * sizeof(float) + (kMma ? kWeightBytes : 0);
     static bool configured = false;                     // per instantiation
     if (!configured) {
         NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma, kMode>,
