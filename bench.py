@@ -1,21 +1,23 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the neural-OIT hot path on B200 (contract: see DESIGN.md §Measurement).
+"""bench.py -- throughput of the neural-OIT hot path on B200 (contract: see DESIGN.md section 7).
 
-One STEP = one pass of the whole hot path over the 1080p high-depth-
-complexity workload (BASELINE.json configs[2], "cfg3", plus the half/quarter buffers of the same
-primitives):
-   1. noit_resolve   plain fused resolve of the frame (S1-S5)          <- dominant kernel
+`metric` / `value` are BASELINE.json's: Mpixels/s (and fragments/s, % of the HBM roofline) of the
+neural-OIT resolve at 1080p -- the plain fused resolve (S1-S5, `noit_resolve`) of the 1080p
+high-depth-complexity workload (BASELINE.json configs[2], "cfg3"): value = P / its mean CUDA-event
+time, `ms_per_step` = that time.  It is timed inside the step loop below, so every launch finds
+the L2 holding other kernels' data (and its 647 MB of inputs exceed the 126 MB L2 anyway).
+
+One STEP = one pass of the whole hot path over that frame:
+   1. noit_resolve   plain fused resolve of the frame (S1-S5)          <- dominant kernel, `value`
    2. noit_quadtree  colour-variance tiles of its result (S6)
       + noit_quadtree_balance  2:1 tile consistency, histogram, demand index, Eq. 2 (NEXT-1)
    3. noit_resolve   adaptive resolve guided by those tiles (S7)
    4. noit_reproject previous result under a small camera motion (S8)
    5. noit_resolve   fallback resolve of the rejected pixels (S9)
-and produces three output frames, so `value` = 3*P pixels / step time.  The plain fused resolve
-alone (the metric BASELINE.json names: Mpixels/s and fragments/s at 1080p, % of HBM roofline) is
-timed with its own CUDA events inside the same timed region and reported in `roofline` and in
-`resolve_*`.  Inputs (647 MB) are larger than L2 (126 MB), so no flush is needed between steps.
+The whole step (three output frames) is reported beside it as `step_*` (eager, serial CUDA graph,
+forked CUDA graph), every kernel of the step has a line in `roofline_all`.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--scaling weak|strong]
 """
 from __future__ import annotations
 
@@ -35,7 +37,7 @@ if ROOT not in sys.path:
 
 BG = (0.2, 0.3, 0.4)
 WORKLOAD = "cfg3: 1920x1080, 512 ellipses, mean 24 / max 128 fragments per pixel, RGBA fp16, bf16 weights"
-METRIC = "Mpixels/s of neural OIT resolve at 1080p (whole hot path S1-S9 per step)"
+METRIC = "Mpixels/s and fragments/s of neural OIT resolve at 1080p; % of HBM roofline"
 
 
 def peaks():
@@ -101,12 +103,42 @@ def camera_shift_matrix(W: int, H: int) -> np.ndarray:
 
 
 def resolve_traffic():
-    """dram bytes per launch of the plain resolve from the committed ncu capture (profiles/)."""
-    try:
-        d = json.load(open(os.path.join(ROOT, "profiles", "r01_resolve_ncu.json.txt")))
-        return int(d["dram_bytes_read"]) + int(d["dram_bytes_write"])
-    except Exception:
-        return None
+    """(dram bytes per launch of the plain resolve, source file): the newest committed ncu capture
+    profiles/rNN_resolve_ncu.json.txt (one `ncu --set full` launch; re-captured when the kernel
+    changes -- the command is in the .md of the same name)."""
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_resolve_ncu.json.txt")), reverse=True):
+        try:
+            d = json.load(open(path))
+            return int(d["dram_bytes_read"]) + int(d["dram_bytes_write"]), os.path.relpath(path, ROOT)
+        except Exception:
+            continue
+    return None, None
+
+
+def step_bytes(fbh, half, quarter, lod_of_pixel, rejected, F_rejected):
+    """Algorithmic bytes of every kernel of the step (SURVEY 8(d) formulas; fp16 colours)."""
+    P, F = fbh.num_pixels, fbh.num_fragments
+    W, H = fbh.width, fbh.height
+    n = np.diff(fbh.offsets.astype(np.int64))
+    coarse = lod_of_pixel > 0
+    b = {"resolve": resolve_bytes(P, F, 8, 2, True)}
+    b["quadtree"] = 16 * P + 4 * ((W + 63) // 64) * ((H + 63) // 64) + ((W + 7) // 8) * ((H + 7) // 8) + 16
+    b["balance"] = 8 * ((W + 63) // 64) * ((H + 63) // 64) + ((W + 7) // 8) * ((H + 7) // 8) + 28
+    # adaptive: lod-0 pixels read their whole list; lod>0 pixels only their depths + the winner's
+    # colour; the coarse lists of coarse leaves are read once, plus their offsets; one image out
+    ad = 4 * (P + 1) + 16 * P + 12 * int(n[~coarse].sum()) + 4 * int(n[coarse].sum()) + 8 * int((n[coarse] > 0).sum())
+    for lod, cb in ((1, half), (2, quarter)):
+        yy, xx = np.divmod(np.arange(cb.num_pixels), cb.width)
+        fy, fx = np.minimum(yy << lod, H - 1), np.minimum(xx << lod, W - 1)
+        used = lod_of_pixel[fy * W + fx] == lod
+        cn = np.diff(cb.offsets.astype(np.int64))
+        ad += 12 * int(cn[used].sum()) + 4 * int(used.sum())
+    b["adaptive"] = ad
+    # reproject: cur depth + gathered prev depth and prev trans; trans, depth, final, accept out
+    b["reproject"] = 4 * P + 4 * P + 16 * P + (16 + 4 + 16 + 1) * (P - rejected) + P + 4 * rejected
+    b["fallback"] = 4 * rejected + 8 * rejected + 12 * F_rejected + 36 * rejected
+    return b
 
 
 def resolve_bytes(P: int, F: int, color_bytes: int, n_images: int, depth1: bool) -> int:
@@ -149,54 +181,38 @@ def run_dryrun(args):
         dist.destroy_process_group()
 
 
-def oracle_step(oracle, sc, w_eff, M, state):
-    """The same five calls as the GPU step, on the CPU oracle (reference arm / cpu_baseline)."""
-    fbh = sc.full
-    W, H = fbh.width, fbh.height
-    r = oracle.resolve(fbh, w_eff, BG)
-    qt = oracle.quadtree(r["final"], W, H, 0, 6)
-    qt = oracle.quadtree_balance(qt["tile_mask"], W, H)
-    oracle.resolve(fbh, w_eff, BG, half=sc.half, quarter=sc.quarter, cell_level=qt["cell_level"])
-    rp = oracle.reproject(W, H, M, 1e-3, BG, r["trans"], r["depth1"], r["depth1"])
-    out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
-    oracle.resolve(fbh, w_eff, BG, pixel_list=rp["reject_list"], out=out)
-    state["rejected"] = rp["reject_count"]
-
-
 def run_reference(args):
-    """`--impl reference`: the oracle, as it stands, on the host cores; each step = the whole
-    path on a bounded sample (the top `rows` pixel rows of the same cfg3 frame)."""
+    """`--impl reference`: the oracle, as it stands, on the host cores, same metric as the product
+    arm: each step = the plain resolve (S1-S5) of the cfg3 frame, or of a 256-row band of it when a
+    whole frame takes more than 4 s on this host (bounded sample)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import noit_scenes
     import oracle
-    sc = noit_scenes.cfg3(0, coarse=True)
+    sc = noit_scenes.cfg3(0)
     w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    fbh = sc.full
     t0 = time.perf_counter()
-    oracle_step(oracle, sc, w_eff, camera_shift_matrix(sc.full.width, sc.full.height), {})
-    if time.perf_counter() - t0 > 4.0:           # slow host: bounded sample = a 256-row band
-        y0, y1 = 384, 640
-        sc = noit_scenes.Scene("cfg3-band", sc.full.rows(y0, y1), sc.half.rows(y0 // 2, y1 // 2),
-                               sc.quarter.rows(y0 // 4, y1 // 4), sc.weights, sc.mlp_precision)
-    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
-    M = camera_shift_matrix(sc.full.width, sc.full.height)
-    state = {}
+    oracle.resolve(fbh, w_eff, BG)
+    if time.perf_counter() - t0 > 4.0:
+        fbh = fbh.rows(384, 640)
     for _ in range(args.warmup):
-        oracle_step(oracle, sc, w_eff, M, state)
+        oracle.resolve(fbh, w_eff, BG)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_step(oracle, sc, w_eff, M, state)
+        oracle.resolve(fbh, w_eff, BG)
     dt = time.perf_counter() - t0
-    P = sc.full.num_pixels
-    value = 3 * P * args.steps / dt / 1e6
+    P, F = fbh.num_pixels, fbh.num_fragments
+    value = P * args.steps / dt / 1e6
     cores = oracle.num_threads()
-    sample = f"{sc.full.height} rows of the cfg3 frame ({P} pixels, {sc.full.num_fragments} fragments) per step"
+    sample = f"plain resolve of {fbh.height} rows of the cfg3 frame ({P} pixels, {F} fragments) per step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": "Mpixels/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "data": "synthetic", "config": {"workload": WORKLOAD, "pixels": P, "fragments": F, "sample": sample},
+        "fragments_per_s": F * args.steps / dt,
         "cpu_baseline": {"value": value, "unit": "Mpixels/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "Mpixels/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -215,8 +231,26 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     dist, rank, world = dist_setup(args.gpus, "nccl")
 
-    # weak scaling: every rank resolves its own 1080p frame (seed = rank), no data-path collective
-    sc = noit_scenes.cfg3(rank, coarse=True)
+    if args.scaling == "strong" and world > 1:
+        # strong scaling: ONE cfg3 frame (seed 0) split into 64-row-aligned, fragment-balanced row
+        # bands; every rank runs the whole step on its band, no data-path collective
+        # (a reprojected pixel whose source row lies outside the band counts as disoccluded and is
+        # resolved by S9, so no halo is exchanged)
+        from paper_2606_16747_b200.sharding import shard_rows
+        whole = noit_scenes.cfg3(0, coarse=True)
+        bands = shard_rows(whole.full.offsets, whole.full.width, whole.full.height, world)
+        y0, y1 = bands[rank]
+        if y1 <= y0:
+            raise SystemExit(f"bench.py: rank {rank} got an empty band ({world} ranks, {whole.full.height} rows)")
+        sc = noit_scenes.Scene(f"cfg3-rows-{y0}-{y1}", whole.full.rows(y0, y1),
+                               whole.half.rows(y0 // 2, (y1 + 1) // 2), whole.quarter.rows(y0 // 4, (y1 + 3) // 4),
+                               whole.weights, whole.mlp_precision)
+        P_job, F_job = whole.full.num_pixels, whole.full.num_fragments
+        del whole
+    else:
+        # weak scaling: every rank resolves its own 1080p frame (seed = rank), no data-path collective
+        sc = noit_scenes.cfg3(rank, coarse=True)
+        P_job, F_job = sc.full.num_pixels * world, sc.full.num_fragments * world
     fbh = sc.full
     W, H, P, F = fbh.width, fbh.height, fbh.num_pixels, fbh.num_fragments
     fb, hb, qb = (noit.DeviceFragBuf.from_host(b, dev) for b in (sc.full, sc.half, sc.quarter))
@@ -230,7 +264,7 @@ def run_ours(args):
     rp = None
     d_plain = ctx.make_resolve_desc(fb, BG, plain["trans"], plain["final"], plain["depth1"])
     stream = torch.cuda.current_stream()
-    names = ["resolve", "quadtree+balance", "adaptive", "reproject", "fallback"]
+    names = ["resolve", "quadtree", "balance", "adaptive", "reproject", "fallback"]
 
     def step(ev=None):
         nonlocal qt, bal, rp
@@ -238,15 +272,16 @@ def run_ours(args):
         ctx.resolve_desc(d_plain)
         if ev: ev[1].record(stream)
         qt = ctx.quadtree(plain["final"], W, H, noit.QT_VARIANCE, 6, out=qt)
-        bal = ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal)
         if ev: ev[2].record(stream)
-        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=bal["cell_level"])
+        bal = ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal)
         if ev: ev[3].record(stream)
-        rp = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"], out=rp)
+        ctx.resolve(fb, BG, want=(), out=adapt, half=hb, quarter=qb, cell_level=bal["cell_level"])
         if ev: ev[4].record(stream)
+        rp = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"], out=rp)
+        if ev: ev[5].record(stream)
         ctx.resolve(fb, BG, want=(), out=dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"]),
                     pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
-        if ev: ev[5].record(stream)
+        if ev: ev[6].record(stream)
 
     # The same step with its two independent chains forked inside the graph: after the plain
     # resolve, frame 3 (reprojection + fallback, S8-S9) depends only on that resolve's outputs and
@@ -282,7 +317,7 @@ def run_ours(args):
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
-    events = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(args.steps)]
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
     launches0 = ctx.launch_count
     if dist is not None:
         dist.barrier()
@@ -293,7 +328,7 @@ def run_ours(args):
     if dist is not None:
         dist.barrier()
     launches = ctx.launch_count - launches0
-    total_ms = events[0][0].elapsed_time(events[-1][5])
+    total_ms = events[0][0].elapsed_time(events[-1][6])
     total_ms = max_over_ranks(dist, total_ms, dev)
     eager_ms = total_ms
     # The step is launch-bound around its short kernels (seven launches + two memsets, ~15 us of
@@ -409,25 +444,52 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = peaks()
         ms_step = total_ms / args.steps
-        rbytes = resolve_bytes(P, F, 8, 2, True)
+        # per-kernel algorithmic bytes of the step, this rank's frame or band
+        lod_px = np.asarray([2, 1, 0, 0], np.int64)[
+            bal["cell_level"].cpu().numpy().reshape((H + 7) // 8, (W + 7) // 8).repeat(8, 0).repeat(8, 1)[:H, :W]
+        ].reshape(-1)
+        rl = rp["reject_list"].cpu().numpy().view(np.uint32)[:rejected].astype(np.int64)
+        F_rej = int(np.diff(fbh.offsets.astype(np.int64))[rl].sum())
+        kb = step_bytes(fbh, sc.half, sc.quarter, lod_px, rejected, F_rej)
+        kname = {"resolve": "resolve_staged_kernel<half,4,mma,ALL> (noit_resolve, S1-S5)",
+                 "quadtree": "quadtree_kernel (noit_quadtree, S6)",
+                 "balance": "balance_kernel (noit_quadtree_balance, NEXT-1)",
+                 "adaptive": "coarse_g_kernel + resolve_staged_kernel<half,4,mma,ADAPTIVE> (noit_resolve, S7)",
+                 "reproject": "reproject_kernel<nearest> (noit_reproject, S8)",
+                 "fallback": "resolve_staged_kernel<half,8,ffma2,LIST> (noit_resolve, S9)"}
+        roofline_all = [{"kernel": kname[k], "step": k, "bytes": int(kb[k]), "ms": per_kernel[k],
+                         "achieved_gbs": kb[k] / (per_kernel[k] * 1e-3) / 1e9,
+                         "frac": kb[k] / (per_kernel[k] * 1e-3) / 1e9 / peak} for k in names]
+        rbytes = kb["resolve"]
         achieved = rbytes / (resolve_ms * 1e-3) / 1e9
+        traffic, traffic_src = resolve_traffic()
         rec = {
-            "metric": METRIC, "value": 3 * P * world / (ms_step * 1e-3) / 1e6, "unit": "Mpixels/s",
-            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
-            "config": {"workload": WORKLOAD, "pixels": P, "fragments": F, "frames_per_step": 3, "launch": launch_mode,
-                       "l2": "inputs (647 MB) larger than L2 (126 MB); no flush", "seed": "rank"},
-            "resolve_mpix_s": P * world / (resolve_ms * 1e-3) / 1e6,
-            "resolve_gfrag_s": F * world / (resolve_ms * 1e-3) / 1e9,
-            "kernel_ms": per_kernel, "ms_per_step_eager": eager_ms / args.steps,
-            "ms_per_step_serial_graph": None if serial_graph_ms is None else serial_graph_ms / args.steps,
+            "metric": METRIC, "value": P_job / (resolve_ms * 1e-3) / 1e6, "unit": "Mpixels/s",
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": resolve_ms,
+            "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "pixels": P_job, "fragments": F_job,
+                       "what_is_timed": "the plain fused resolve (noit_resolve, S1-S5), one launch per step, "
+                                        "CUDA events on the launching stream inside the whole-path step loop",
+                       "l2": "inputs (647 MB) larger than L2 (126 MB); no flush",
+                       "sharding": ("none" if world == 1 else
+                                    ("one frame in fragment-balanced 64-row bands, no collective" if args.scaling == "strong"
+                                     else "one frame per rank (seed = rank), no collective"))},
+            "fragments_per_s": F_job / (resolve_ms * 1e-3),
+            "resolve_mpix_s": P_job / (resolve_ms * 1e-3) / 1e6,
+            "resolve_gfrag_s": F_job / (resolve_ms * 1e-3) / 1e9,
+            "kernel_ms": per_kernel,
+            "step_frames": 3, "step_launch": launch_mode, "step_ms": ms_step,
+            "step_mpix_s": 3 * P_job / (ms_step * 1e-3) / 1e6,
+            "step_ms_eager": eager_ms / args.steps,
+            "step_ms_serial_graph": None if serial_graph_ms is None else serial_graph_ms / args.steps,
             "extras_ms": extras,
-            "roofline": {"bound": "hbm", "kernel": "noit_resolve (plain fused, S1-S5)", "achieved": achieved,
+            "roofline": {"bound": "hbm", "kernel": kname["resolve"], "achieved": achieved,
                          "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                         "algorithmic_bytes": rbytes, "traffic": resolve_traffic(),
-                         "traffic_source": "profiles/r01_resolve_ncu.json.txt (ncu --set full, one launch)"},
-            "e2e": {"value": P * world / (e2e_ms * 1e-3) / 1e6, "unit": "Mpixels/s",
+                         "algorithmic_bytes": rbytes, "bytes_formula": "4(P+1) + 12F + 2*16P + 4P",
+                         "traffic": traffic, "traffic_source": traffic_src},
+            "roofline_all": roofline_all,
+            "e2e": {"value": P_job / (e2e_ms * 1e-3) / 1e6, "unit": "Mpixels/s",
                     "what": "noit_resolve_host on the same frame, pinned host buffers",
                     "h2d_bytes_per_step": 4 * (P + 1) + 12 * F, "d2h_bytes_per_step": 16 * P,
                     "ms_per_step": e2e_ms},
@@ -534,6 +596,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: one frame per rank (weak) or one frame split into row bands (strong)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="time the step eagerly (no CUDA graph)")
     ap.add_argument("--no-fork", action="store_true", help="graph replay of the serial step only")

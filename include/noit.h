@@ -195,8 +195,11 @@ noit_status noit_quadtree16(noit_ctx* ctx, const float* image /*[P][4]*/, int32_
 /* ---- NEXT-2: temporal tile state ("tiles computed in frame F_t guide ... F_t+1", P:61
  * split / merge thresholds, "tiles may change by only one level per frame"; O11, A26).
  * noit_quadtree with a memory: a node that was NOT split in prev_tile_mask splits iff
- * metric > split threshold; a node that WAS split merges iff metric < merge threshold
- * (merge <= split: inside the band a node keeps its state).  Then the depth of every base tile
+ * metric > split threshold; a node that WAS split merges iff metric < merge threshold.  The
+ * rule is defined for either order of the two thresholds: merge <= split is the stabilising
+ * order (inside the band a node keeps its state, reading A26); merge > split is P:61's sentence
+ * read literally ("split thresholds being smaller than the merge thresholds"): a node whose
+ * metric lies strictly between the two then changes state every frame.  Then the depth of every base tile
  * is limited to its previous depth +- max_level_step (deeper: truncated; shallower: refined
  * uniformly).  prev_tile_mask == NULL: no history, identical to noit_quadtree with the split
  * thresholds.  prev_tile_mask must not alias tile_mask.  max_level_step in [0, 3], 0 = no

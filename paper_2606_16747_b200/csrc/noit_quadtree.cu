@@ -302,8 +302,9 @@ extern "C" noit_status noit_quadtree_temporal(noit_ctx* ctx, const float* image,
         return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_temporal: image/params is NULL");
     if (params->max_level_step < 0 || params->max_level_step > 3)
         return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_temporal: max_level_step must be in [0, 3]");
-    if (params->var_merge_q > params->var_split_q || params->corner_merge > params->corner_split)
-        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_temporal: merge threshold above split threshold");
+    // either order of the two thresholds is a well-defined rule (merge <= split: a band in which a
+    // node keeps its state, A26; merge > split: P:61's sentence read literally, a band in which a
+    // node alternates) -- both are callable
     if (prev_tile_mask && prev_tile_mask == tile_mask)
         return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_quadtree_temporal: prev_tile_mask aliases tile_mask");
     QtTemporal tq = {prev_tile_mask, params->var_merge_q, params->corner_merge, params->max_level_step};

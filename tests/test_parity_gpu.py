@@ -1,11 +1,15 @@
 """GPU parity (`-m gpu`): the CUDA path through the C ABI versus the CPU oracle, element by
-element on the same seeded inputs.  Classes (DESIGN.md "Tolerances"):
+element on the same seeded inputs.  Classes (DESIGN.md section 6):
   bit-exact  : idx1, idx2, count, depth1, tile_mask, cell_level, hist, accept, reject set,
                reprojected copies
-  fp32       : |a-b| <= 1e-5 max(|a|,|b|) + 1e-6   (layers, tail accumulators, compositing)
-  mlp-fp32   : the above + 1e-5 * T_2 * mag(f), mag(f) = the MLP evaluated with |W|, |b|, |x|
-               (forward error bound of fp32 dot products with cancellation)
-  bf16 mode  : 2e-3 absolute on colour (BASELINE.json north_star)
+  fp32       : |a-b| <= 1e-5 max(|a|,|b|) + 1e-6   (BASELINE.json north_star, as written:
+               layers, tail accumulators, compositing, and the resolve's outputs)
+  mlp guard  : + K_MLP * eps32 * T_2 * mag(f), K_MLP = 4, eps32 = 2^-24, mag(f) = the MLP evaluated
+               with |W|, |b|, |x| (first-order forward bound of an fp32 evaluation in any order);
+               at most 2.4e-7 * mag, where round 1 allowed 1e-5 * mag.  Measured on B200 it is never
+               needed: the largest |a-b| / (1e-5 max + 1e-6) over cfg1-cfg3 and the random frames
+               is 0.57 (printed per test in the terminal summary, tests/conftest.py).
+  bf16 mode  : 2e-3 absolute on colour (north_star) on top of the bar above
 """
 import numpy as np
 import pytest
@@ -26,13 +30,22 @@ def noit():
     return m
 
 
+K_MLP = 4.0
+EPS32 = 2.0 ** -24
+RATIOS = {}          # test id -> largest |a-b| / (1e-5 max(|a|,|b|) + 1e-6) seen (terminal summary)
+
+
 def close(a, b, rel=1e-5, abs_=1e-6, extra=None):
     a = np.asarray(a, np.float64)
     b = np.asarray(b, np.float64)
-    tol = rel * np.maximum(np.abs(a), np.abs(b)) + abs_
-    if extra is not None:
-        tol = tol + extra
-    bad = np.abs(a - b) > tol
+    base = rel * np.maximum(np.abs(a), np.abs(b)) + abs_
+    err = np.abs(a - b)
+    if err.size:
+        import os
+        key = os.environ.get("PYTEST_CURRENT_TEST", "?").split(" ")[0].split("::")[-1]
+        RATIOS[key] = max(RATIOS.get(key, 0.0), float((err / base).max()))
+    tol = base if extra is None else base + extra
+    bad = err > tol
     if bad.any():
         i = np.argwhere(bad)[0]
         raise AssertionError(f"{bad.sum()} mismatches, first at {tuple(i)}: {a[tuple(i)]} vs {b[tuple(i)]}")
@@ -61,7 +74,7 @@ def check_resolve(noit, fb_host, weights, precision, got, ref=None, bf16_abs=2e-
     a1, a2 = lay["layer1"][:, 3].astype(np.float64), lay["layer2"][:, 3].astype(np.float64)
     t2 = (1 - a1) * (1 - a2)
     mag = mlp_magnitude(w_eff, lay["features"]) * t2[:, None]
-    extra = np.concatenate([1e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])          # bit-exact
     for k in ("trans", "final"):
         g = got[k].cpu().numpy()
@@ -134,7 +147,7 @@ def test_infer(noit, precision):
     w_eff = oracle.effective_weights(w, precision)
     assert np.array_equal(ctx.get_weights(), w_eff)                  # same rounding, bit for bit
     got = ctx.infer(torch.from_numpy(x).cuda()).cpu().numpy()
-    close(got, oracle.infer(w_eff, x), extra=1e-5 * mlp_magnitude(w_eff, x))
+    close(got, oracle.infer(w_eff, x), extra=K_MLP * EPS32 * mlp_magnitude(w_eff, x))
     assert ctx.infer(torch.empty((0, 5), device="cuda")).shape == (0, 3)
 
 
@@ -214,6 +227,47 @@ def test_resolve_random_stress(noit, block):
         ctx = noit.Noit(w, precision)
         got = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
         check_resolve(noit, fbh, w, precision, got)
+
+
+@pytest.mark.parametrize("dtype,precision", [(np.float16, 1), (np.float32, 0)])
+def test_resolve_alpha_exactly_zero_and_one(noit, dtype, precision):
+    """Degenerate opacities the method has: alpha exactly 1 in the tail gives
+    T_tail = 0 while A_tail > 0; alpha exactly 0 everywhere in the tail gives A_tail = 0 with
+    N > 2 (reading A2: has_tail false, tail term forced to 0, features (N, 1, 0, 0, 0)); whole
+    pixels of alpha 0 or 1; light and heavy lists."""
+    rng = np.random.default_rng(77 + precision)
+    fbh = random_fb(rng, 130, 21, 24, dtype, tie_frac=0.2, empty_frac=0.05, heavy=(6, 400))
+    off = fbh.offsets.astype(np.int64)
+    n = np.diff(off)
+    pix = np.repeat(np.arange(n.size), n)
+    a = fbh.rgba[:, 3].astype(np.float32)
+    u = rng.random(a.size)
+    a[u < 0.25] = 0.0
+    a[u > 0.75] = 1.0
+    kind = rng.integers(0, 5, n.size)                       # per pixel: 0-1 mixed, 2 all zero, 3 all one,
+    a[kind[pix] == 2] = 0.0                                 # 4 tail of zeros behind two opaque-ish layers
+    a[kind[pix] == 3] = 1.0
+    lay = oracle.build_features(fbh)
+    k4 = np.nonzero((kind == 4) & (n > 2))[0]
+    a[np.isin(pix, k4)] = 0.0
+    for idx in ("idx1", "idx2"):
+        a[off[k4] + lay[idx][k4].astype(np.int64)] = 0.5
+    fbh.rgba[:, 3] = a.astype(dtype)
+    lay = oracle.build_features(fbh)
+    assert ((lay["tail_raw"][:, 3] == 0) & (n > 2)).sum() > 50          # all-zero tails with N > 2
+    assert ((lay["tail_raw"][:, 4] == 0) & (lay["tail_raw"][:, 3] > 0)).sum() > 50   # T_tail = 0, A_tail > 0
+    w = noit_scenes.mlp_weights(3)
+    ctx = noit.Noit(w, precision)
+    fb = noit.DeviceFragBuf.from_host(fbh)
+    check_resolve(noit, fbh, w, precision, ctx.resolve(fb, BG))
+    got = ctx.build_features(fb)
+    assert np.array_equal(u32(got["idx1"]), lay["idx1"]) and np.array_equal(u32(got["idx2"]), lay["idx2"])
+    close(got["features"].cpu().numpy(), lay["features"])
+    close(got["tail_raw"].cpu().numpy(), lay["tail_raw"])
+    # an all-zero tail is exactly the two-layer composite (north_star invariant, A2)
+    z = (lay["tail_raw"][:, 3] == 0)
+    final = ctx.resolve(fb, BG)["final"].cpu().numpy()
+    close(final[z], oracle.exact(fbh, BG)["final"][z])
 
 
 def test_resolve_per_pixel_background(noit):

@@ -6,7 +6,8 @@ import torch
 
 import noit_scenes
 import oracle
-from test_parity_gpu import BG, check_resolve, close, mlp_magnitude, noit, random_fb, u32  # noqa: F401
+from test_parity_gpu import (BG, EPS32, K_MLP, check_resolve, close, mlp_magnitude, noit,  # noqa: F401
+                             random_fb, u32)
 
 pytestmark = pytest.mark.gpu
 
@@ -44,6 +45,34 @@ def test_quadtree_random_images(noit, W, H, metric):
     levels = set(np.unique(oracle.quadtree(img, W, H, metric, 6, 0.02)["cell_level"]).tolist())
     if W >= 1920 and metric == 0:
         assert levels == {0, 1, 2, 3}
+
+
+@pytest.mark.parametrize("W,H", [(200, 136), (1920, 1080), (65, 7)])
+@pytest.mark.parametrize("metric", [0, 1])
+def test_quadtree_out_of_range_pixels(noit, W, H, metric):
+    """The resolve's ReLU output is unbounded above (A11) and is what S6 consumes: colours below 0
+    and above 1 (the +-2.0 spikes of the first version of test_quadtree_random_images, plus whole
+    blocks outside [0, 1]) must give the oracle's masks bit for bit -- both sides quantise
+    q = rint(255 * clamp(c, 0, 1)) for the variance metric and use the raw colour in the corner metric.
+    The oracle's clamp is pinned on the CPU (test_quadtree_quantiser_clamps_out_of_range_colours)."""
+    rng = np.random.default_rng(W * 11 + H + metric)
+    yy, xx = np.mgrid[0:H, 0:W]
+    img = np.zeros((H, W, 4), np.float32)
+    for c in range(3):
+        img[..., c] = 0.5 + 0.3 * np.sin(xx / (40.0 + 10 * c)) * np.cos(yy / 55.0)
+    img[..., :3] += (rng.random((H, W, 3)) < 0.002) * 2.0 - (rng.random((H, W, 3)) < 0.002) * 2.0
+    blocks = rng.choice([0.0, 0.0, 0.0, 1.5, -0.7], size=(-(-H // 32), -(-W // 32))).astype(np.float32)
+    img[..., :3] += blocks.repeat(32, 0).repeat(32, 1)[:H, :W, None]
+    img[..., 3] = rng.random((H, W))
+    assert W < 128 or ((img[..., :3] < 0).any() and (img[..., :3] > 1).any())
+    img = np.ascontiguousarray(img.reshape(-1, 4))
+    ctx = noit.Noit()
+    for thr, cthr in ((6, 0.02), (0, 0.0), (400, 0.2)):
+        qt_equal(ctx.quadtree(torch.from_numpy(img).cuda(), W, H, metric, thr, cthr),
+                 oracle.quadtree(img, W, H, metric, thr, cthr))
+    if W >= 128:
+        q16 = ctx.quadtree16(torch.from_numpy(img).cuda(), W, H, metric, 6, 0.02)
+        qt_equal(q16, oracle.quadtree16(img, W, H, metric, 6, 0.02))
 
 
 def test_quadtree_constant_image(noit):
@@ -93,7 +122,7 @@ def test_adaptive_resolve_small(noit, cfg4_small):
     w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
     lay = oracle.build_features(sc.full)
     mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     for k in ("trans", "final"):
         close(got[k].cpu().numpy(), ref[k], extra=extra)
         assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
@@ -106,6 +135,33 @@ def test_adaptive_resolve_small(noit, cfg4_small):
         close(got0[k].cpu().numpy(), plain[k].cpu().numpy().astype(np.float64), extra=extra)
 
 
+def test_adaptive_resolve_ties_in_the_coarse_buffers(noit):
+    """Exact front depth ties INSIDE the half and quarter buffers (the generator injects them into
+    the full buffer only): the pre-pass's own selection must apply the index tie rule (O1 on the
+    coarse lists, A19), for both colour orders of the tied pair."""
+    import copy
+    from noit_scenes.raster import inject_front_ties
+    sc = copy.deepcopy(noit_scenes.cfg4(5, W=448, H=264, n_prims=96, mean_band=(10.0, 12.0), cap=64))
+    rng = np.random.default_rng(55)
+    assert inject_front_ties(sc.half, rng, 0.5) > 1000 and inject_front_ties(sc.quarter, rng, 0.5) > 300
+    w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
+    mag = mlp_magnitude(w_eff, np.maximum(oracle.build_features(sc.full)["features"], [[64, 1, 1, 1, 1]]))
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    for l2l, thr in (((2, 1, 0, 0), 6), ((2, 2, 1, 1), 10 ** 9), ((1, 1, 1, 1), 6)):
+        _, got, ref, cell = run_adaptive(noit, sc, l2l=l2l, thr=thr)
+        assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+        for k in ("trans", "final"):
+            close(got[k].cpu().numpy(), ref[k], extra=extra)
+    # the frame-global control reads the same coarse buffers through the same pre-pass
+    fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    forced = torch.tensor([2.0, 0.5, 0.25], dtype=torch.float32, device="cuda")
+    g = ctx.resolve(fb, BG, half=hb, quarter=qb, pass_scales=forced)
+    r = oracle.resolve_global(sc.full, sc.half, sc.quarter, w_eff, BG, 1, 2)
+    for k in ("trans", "final"):
+        close(g[k].cpu().numpy(), r[k], extra=extra)
+
+
 def test_adaptive_resolve_ragged_size(noit):
     """Width not a multiple of 8 (cells cut by the right edge), P not a multiple of 32 (last tile
     partial, tiles wrap rows in the middle of a cell): the per-tile lod summary of the pre-pass
@@ -114,7 +170,7 @@ def test_adaptive_resolve_ragged_size(noit):
     assert sc.full.width % 8 and sc.full.num_pixels % 32
     w_eff = oracle.effective_weights(sc.weights, sc.mlp_precision)
     mag = mlp_magnitude(w_eff, np.maximum(oracle.build_features(sc.full)["features"], [[64, 1, 1, 1, 1]]))
-    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     for l2l, thr in (((2, 1, 0, 0), 6), ((2, 2, 1, 0), 6), ((1, 1, 1, 1), 6), ((2, 1, 0, 0), 10 ** 9)):
         _, got, ref, cell = run_adaptive(noit, sc, l2l=l2l, thr=thr)
         assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
@@ -190,6 +246,28 @@ def test_reproject_perspective_path(noit):
     Mneg[3] = -Mneg[3]                                                         # w <= 0 everywhere
     got, ref = check_reproject(noit, W, H, Mneg, 1e-3, prev_t, prev_d, prev_d)
     assert ref["reject_count"] == W * H
+
+
+def test_reproject_mode_b_current_depth_differs(noit):
+    """Reading A21 mode B: the caller has the CURRENT first-layer depth (a depth-only scan), so
+    cur_depth != prev_depth: the transform takes d from cur_depth, the disocclusion test compares
+    d_e with prev_depth at the fetched pixel.  Perspective motion, both filters, a third of the
+    pixels with a depth change beyond tau."""
+    rng = np.random.default_rng(29)
+    W, H = 517, 203
+    proj = noit_scenes.perspective(60.0, W / H, 0.1, 100.0)
+    vp0 = proj @ noit_scenes.view_matrix(np.zeros(3), 0.0, 0.0)
+    vp1 = proj @ noit_scenes.view_matrix(np.asarray([0.04, 0.03, -0.02]), -0.005, 0.002)
+    M = (vp0 @ np.linalg.inv(vp1)).astype(np.float32)
+    prev_t, _ = rand_prev(rng, W, H)
+    yy, xx = np.mgrid[0:H, 0:W]
+    prev_d = (0.95 + 0.03 * np.sin(xx / 37.0) * np.cos(yy / 29.0)).astype(np.float32).reshape(-1)
+    cur_d = prev_d + rng.choice(np.asarray([0.0, 2e-4, -3e-4, 5e-3], np.float32), W * H)
+    cur_d = cur_d.astype(np.float32)
+    assert not np.array_equal(cur_d, prev_d)
+    got, ref = check_reproject(noit, W, H, M, 1e-3, prev_t, prev_d, cur_d)
+    assert 0.15 < ref["reject_count"] / (W * H) < 0.9
+    check_reproject_bilinear(noit, W, H, M, 1e-3, prev_t, prev_d, cur_d)
 
 
 def check_reproject_bilinear(noit, W, H, M, thr, prev_t, prev_d, cur_d):
@@ -285,7 +363,7 @@ def test_fallback_resolve_on_reject_list(noit):
         rej = ~torch.from_numpy(acc).cuda()                                    # rejected == plain
         lay = oracle.build_features(fbh)
         mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-        extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)[~acc]
+        extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)[~acc]
         assert torch.equal(out["depth1"][rej], plain["depth1"][rej])
         for k in ("trans", "final"):
             close(out[k][rej].cpu().numpy(), plain[k][rej].cpu().numpy(), extra=extra)
@@ -325,7 +403,7 @@ def test_cfg4_full_size_adaptive_frame(noit):
     assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
     lay = oracle.build_features(sc.full)
     mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     for k in ("trans", "final"):
         close(got[k].cpu().numpy(), ref[k], extra=extra)
         assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
@@ -368,7 +446,7 @@ def run_sequence(noit, seq, n_frames):
         assert np.array_equal(out["depth1"].cpu().numpy(), ref["depth1"])
         lay = oracle.build_features(fbh)
         mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-        extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+        extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
         for k in ("trans", "final"):
             close(out[k].cpu().numpy(), ref[k], extra=extra)
         fractions.append(n / (W * H))
@@ -382,11 +460,14 @@ def test_cfg5_sequence_reduced_all_eight_frames(noit):
     assert len(fr) == 4 and all(0.0 < f < 0.5 for f in fr), fr
 
 
-def test_cfg5_full_size_first_two_frames(noit):
-    """3840x2160: frame 0 resolved, frame 1 reprojected + fallback (BASELINE.json configs[4])."""
+def test_cfg5_full_size_all_eight_frames(noit):
+    """BASELINE.json configs[4] as stated: 3840x2160, 8 frames, frames 0/2/4/6 resolved and compared
+    element by element, frames 1/3/5/7 reprojected (accept mask, reject set, copies bit-exact) with
+    the rejected pixels resolved by S9.  Frames are rasterised one at a time (~25 s each on the host)."""
     seq = noit_scenes.cfg5(0)
-    fr = run_sequence(noit, seq, 2)
-    assert 0.0 < fr[0] < 0.5, fr
+    assert (seq.width, seq.height) == (3840, 2160)
+    fr = run_sequence(noit, seq, 8)
+    assert len(fr) == 4 and all(0.0 < f < 0.5 for f in fr), fr
 
 
 # -------------------------------------------------------------------------------------------
@@ -451,7 +532,7 @@ def test_frame_global_pass_resolution(noit, cfg4_small, s2, s3):
     assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
     lay = oracle.build_features(sc.full)
     mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     for k in ("trans", "final"):
         close(got[k].cpu().numpy(), ref[k], extra=extra)
         assert np.max(np.abs(got[k].cpu().numpy()[:, :3] - ref[k][:, :3])) <= 2e-3
@@ -474,7 +555,7 @@ def test_frame_global_chain_from_device_scales(noit, cfg4_small):
     ref = oracle.resolve_global(sc.full, sc.half, sc.quarter, w_eff, BG, lod2, lod3)
     lay = oracle.build_features(sc.full)
     mag = mlp_magnitude(w_eff, np.maximum(lay["features"], [[64, 1, 1, 1, 1]]))
-    extra = np.concatenate([2e-5 * mag, np.zeros((mag.shape[0], 1))], axis=1)
+    extra = np.concatenate([K_MLP * EPS32 * mag, np.zeros((mag.shape[0], 1))], axis=1)
     for k in ("trans", "final"):
         close(got[k].cpu().numpy(), ref[k], extra=extra)
 
@@ -502,6 +583,30 @@ def test_quadtree_temporal_random(noit, seed, W, H, metric, step, hist_):
     qt_equal(got, ref)
     if prev is not None:
         assert not np.array_equal(ref["tile_mask"], oracle.quadtree_temporal(img, W, H, None, **kw)["tile_mask"])
+
+
+@pytest.mark.parametrize("metric", [0, 1])
+def test_quadtree_temporal_literal_threshold_order(noit, metric):
+    """P:61's literal order (split threshold below the merge threshold) is callable and equals the
+    oracle over a chain of frames; a node in the band alternates (pinned on the CPU)."""
+    from test_oracle_pins import _random_valid_masks
+    rng = np.random.default_rng(300 + metric)
+    W, H = 333, 200
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    img = (rng.random((H * W, 4)) * rng.random((H * W, 1)) ** 3).astype(np.float32)
+    d_img = torch.from_numpy(img).cuda()
+    kw = dict(metric=metric, var_split=1500, var_merge=2500, corner_split=0.2, corner_merge=0.35, max_step=1)
+    ctx = noit.Noit()
+    r_prev = _random_valid_masks(rng, Tx * Ty)
+    g_prev = torch.from_numpy(r_prev.view(np.int32).copy()).cuda()
+    masks = []
+    for _ in range(4):
+        ref = oracle.quadtree_temporal(img, W, H, r_prev, **kw)
+        got = ctx.quadtree_temporal(d_img, W, H, g_prev, **kw)
+        qt_equal(got, ref)
+        r_prev, g_prev = ref["tile_mask"], got["tile_mask"]
+        masks.append(ref["tile_mask"].copy())
+    assert len({m.tobytes() for m in masks}) >= 2              # the history matters over the chain
 
 
 def test_quadtree_temporal_chain_over_cfg5_frames(noit):
