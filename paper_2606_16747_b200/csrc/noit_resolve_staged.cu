@@ -338,7 +338,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
 // the kernel
 // ------------------------------------------------------------------------------------------
 template <typename ColorT, int L, bool kMma, int kMode>
-__global__ void __launch_bounds__(kWarpsPerCta * 32, kMode == NOIT_RESOLVE_LIST ? 1 : NOIT_X_CTAS)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, kMode == NOIT_RESOLVE_LIST ? 7 : NOIT_X_CTAS)
 resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
 {
     typedef typename Color<ColorT>::Packed Packed;

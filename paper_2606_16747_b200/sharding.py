@@ -48,3 +48,74 @@ def gather_rows(parts: list, bands: list, width: int, height: int, channels: int
     for part, (y0, y1) in zip(parts, bands):
         out[y0 * width:y1 * width] = part.reshape((-1, channels) if channels > 1 else (-1,))
     return out
+
+
+# ---- reprojection across bands (S8): a row halo of the previous frame ----------------------
+def halo_rows(height: int, max_motion: float = 0.02) -> int:
+    """Rows of `prev_trans` / `prev_depth` a band needs from each neighbour so that every source
+    pixel of a reprojection with at most `max_motion` * H of vertical screen motion is local
+    (ceil(0.02 H) + 1; BASELINE.json cfg5: <= 2 % screen motion per frame)."""
+    return int(np.ceil(max_motion * height)) + 1
+
+
+def extended_band(band, halo: int, height: int):
+    """[y0 - halo, y1 + halo) clipped to the frame."""
+    y0, y1 = band
+    return max(0, y0 - halo), min(height, y1 + halo)
+
+
+def band_matrix(M: np.ndarray, height: int, y0: int, y1: int) -> np.ndarray:
+    """Reprojection matrix of the rows [y0, y1) seen as a frame of their own.
+
+    noit_reproject works in the NDC of the buffer it is given (pixel centre y + 0.5 over the
+    buffer's height, y down, A23).  A band's NDC is an affine image of the frame's:
+    y_frame = s * y_band + t with s = (y1 - y0) / H, t = s + 2 y0 / H - 1.  So the band's matrix is
+    G2L . M . L2G (float64 here, cast by the caller), both current and previous buffers being the
+    same rows.  Coordinate bookkeeping only: the transform itself runs in the kernel."""
+    s = (y1 - y0) / height
+    t = s + 2.0 * y0 / height - 1.0
+    l2g = np.eye(4)
+    l2g[1, 1], l2g[1, 3] = s, t
+    g2l = np.eye(4)
+    g2l[1, 1], g2l[1, 3] = 1.0 / s, -t / s
+    return g2l @ np.asarray(M, np.float64) @ l2g
+
+
+def exchange_halo_rows(band_rows, halo: int, rank: int, world_size: int, group=None):
+    """Send this rank's first / last `halo` rows to the neighbouring ranks and receive theirs.
+
+    `band_rows` is a torch tensor [rows, ...] (prev_trans or prev_depth of this rank's band).
+    Returns (above, below): the neighbour rows that precede / follow the band (None at the frame
+    edge).  One send + one receive per neighbour (`torch.distributed` P2P: NCCL moves them over
+    NVLink peer to peer, gloo on the CPU); bands shorter than `halo` rows send what they have.
+    The only data-path exchange of the sharded path, and only reprojection needs it."""
+    import torch
+    import torch.distributed as dist
+    ops, above, below = [], None, None
+    n = band_rows.shape[0]
+    h = min(halo, n)
+    counts = [torch.zeros(1, dtype=torch.int64, device=band_rows.device) for _ in range(2)]
+    # neighbours' band heights may be below `halo`: exchange the row counts first
+    mine = torch.tensor([h], dtype=torch.int64, device=band_rows.device)
+    if rank > 0:
+        ops += [dist.P2POp(dist.isend, mine, rank - 1, group), dist.P2POp(dist.irecv, counts[0], rank - 1, group)]
+    if rank < world_size - 1:
+        ops += [dist.P2POp(dist.isend, mine, rank + 1, group), dist.P2POp(dist.irecv, counts[1], rank + 1, group)]
+    if ops:
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+    ops = []
+    if rank > 0:
+        above = torch.empty((int(counts[0].item()),) + tuple(band_rows.shape[1:]), dtype=band_rows.dtype,
+                            device=band_rows.device)
+        ops += [dist.P2POp(dist.isend, band_rows[:h].contiguous(), rank - 1, group),
+                dist.P2POp(dist.irecv, above, rank - 1, group)]
+    if rank < world_size - 1:
+        below = torch.empty((int(counts[1].item()),) + tuple(band_rows.shape[1:]), dtype=band_rows.dtype,
+                            device=band_rows.device)
+        ops += [dist.P2POp(dist.isend, band_rows[n - h:].contiguous(), rank + 1, group),
+                dist.P2POp(dist.irecv, below, rank + 1, group)]
+    if ops:
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+    return above, below

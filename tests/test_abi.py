@@ -117,3 +117,42 @@ def test_bench_gloo_world2(tmp_path):
     rec = json.loads(lines[0])
     assert rec["n_gpus"] == 2 and rec["dryrun"] is True and rec["scaling"] == "weak"
     assert rec["ranks_seen"] == 2
+
+
+def test_sharded_path_gloo_world2():
+    """SURVEY 8(e) with two real ranks (gloo, CPU): each rank slices ITS band of the same seeded
+    frame (shard_rows / slice_rows), exchanges the reprojection halo with its neighbour
+    (exchange_halo_rows) and rank 0 reassembles per-band results with gather_rows."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", "29741",
+           os.path.join(ROOT, "tests", "gloo_shard_worker.py")]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-3000:]
+    import json
+    rec = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert rec["world"] == 2 and rec["counts_equal"] and rec["first_depth_equal"] and rec["halo_ok"]
+    (a0, a1), (b0, b1) = rec["bands"]
+    assert a0 == 0 and a1 == b0 and b1 == 256 and a1 % 64 == 0 and 0 < a1 < 256
+    f = rec["fragments_per_rank"]
+    assert abs(f[0] - f[1]) <= 0.5 * sum(f)                   # balanced by fragments, 64-row granularity
+
+
+def test_band_matrix_is_the_frame_matrix_in_band_coordinates():
+    """band_matrix: a point of the band, mapped by the band's matrix in the band's NDC, lands where
+    the frame's matrix puts it in the frame's NDC (float64 check of the coordinate bookkeeping)."""
+    from paper_2606_16747_b200.sharding import band_matrix
+    import noit_scenes
+    H, y0, y1 = 1080, 256, 640
+    proj = noit_scenes.perspective(60.0, 16 / 9, 0.1, 100.0)
+    M = (proj @ noit_scenes.view_matrix(np.zeros(3), 0.0, 0.0)) @ np.linalg.inv(
+        proj @ noit_scenes.view_matrix(np.array([0.1, -0.05, 0.2]), 0.01, -0.02))
+    Mb = band_matrix(M, H, y0, y1)
+    rng = np.random.default_rng(0)
+    for _ in range(50):
+        yl, xn, d = rng.uniform(0, y1 - y0), rng.uniform(-1, 1), rng.uniform(0.9, 0.999)
+        c = Mb @ np.array([xn, 2 * (yl + 0.5) / (y1 - y0) - 1, d, 1.0])
+        g = M @ np.array([xn, 2 * (yl + y0 + 0.5) / H - 1, d, 1.0])
+        # previous row inside the band's own frame vs inside the whole frame
+        rb = (c[1] / c[3] + 1) * 0.5 * (y1 - y0) + y0
+        rg = (g[1] / g[3] + 1) * 0.5 * H
+        assert abs(rb - rg) < 1e-9 and abs(c[0] / c[3] - g[0] / g[3]) < 1e-12 and abs(c[2] / c[3] - g[2] / g[3]) < 1e-12

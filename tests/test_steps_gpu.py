@@ -5,6 +5,7 @@ import pytest
 import torch
 
 import noit_scenes
+from noit_scenes.raster import FragBuf
 import oracle
 from test_parity_gpu import (BG, EPS32, K_MLP, check_resolve, close, mlp_magnitude, noit,  # noqa: F401
                              random_fb, u32)
@@ -759,3 +760,88 @@ def test_forked_graph_step_equals_the_eager_step_and_the_oracle(noit, cfg4_small
     oracle.resolve(sc.full, w_eff, BG, pixel_list=rp["reject_list"], out=out)
     close(st["rp"]["final"].cpu().numpy(), out["final"])
 
+
+
+# -------------------------------------------------------------------------------------------
+# the sharded path on one GPU -- a frame resolved band by band equals the whole frame
+# -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_sharded_resolve_and_quadtree_equal_the_whole_frame(noit, world):
+    """Row bands from shard_rows (64-row aligned, fragment balanced), rebased CSR arrays from
+    slice_rows, one resolve + quadtree per band, gather_rows: bit for bit the whole-frame result
+    (every pixel and every 64x64 tile is independent: no exchange)."""
+    from paper_2606_16747_b200.sharding import gather_rows, shard_rows, slice_rows
+    sc = noit_scenes.cfg2(0)
+    fbh = sc.full
+    W, H = fbh.width, fbh.height
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    whole = ctx.resolve(noit.DeviceFragBuf.from_host(fbh), BG)
+    qt_whole = ctx.quadtree(whole["final"], W, H, 0, 6)
+    bands = shard_rows(fbh.offsets, W, H, world)
+    assert bands[0][0] == 0 and bands[-1][1] == H and all(a[1] == b[0] for a, b in zip(bands, bands[1:]))
+    parts = {k: [] for k in ("trans", "final", "depth1")}
+    masks, cells, hist = [], [], np.zeros(4, np.int64)
+    frags = []
+    for (y0, y1) in bands:
+        if y1 == y0:
+            for k in parts:
+                parts[k].append(np.zeros((0, 4) if k != "depth1" else (0,), np.float32))
+            continue
+        off, depth, rgba = slice_rows(fbh.offsets, fbh.depth, fbh.rgba, W, y0, y1)
+        frags.append(int(off[-1]))
+        band = FragBuf(W, y1 - y0, off, depth.copy(), rgba.copy())
+        got = ctx.resolve(noit.DeviceFragBuf.from_host(band), BG)
+        for k in parts:
+            parts[k].append(got[k].cpu().numpy())
+        q = ctx.quadtree(got["final"], W, y1 - y0, 0, 6)
+        masks.append(u32(q["tile_mask"]))
+        cells.append(q["cell_level"].cpu().numpy())
+        hist += u32(q["hist"]).astype(np.int64)
+    for k, ch in (("trans", 4), ("final", 4), ("depth1", 1)):
+        assert np.array_equal(gather_rows(parts[k], bands, W, H, ch), whole[k].cpu().numpy()), k
+    assert np.array_equal(np.concatenate(masks), u32(qt_whole["tile_mask"]))
+    assert np.array_equal(np.concatenate(cells), qt_whole["cell_level"].cpu().numpy())
+    assert np.array_equal(hist, u32(qt_whole["hist"]).astype(np.int64))
+    if world == 2:
+        assert abs(frags[0] - frags[1]) < 0.2 * sum(frags)       # balanced by fragments
+
+
+def test_band_reprojection_with_a_row_halo(noit):
+    """S8 across bands: a band extended by halo_rows(H) rows of its neighbours'
+    prev_trans / prev_depth (here: slices of the whole previous frame stand in for the peer copies
+    exchange_halo_rows makes), reprojected with band_matrix.  Bit-exact against the oracle on the
+    band's inputs, and -- up to fp32 rounding at pixel edges / at the threshold -- the whole-frame
+    reprojection restricted to the band: no pixel is rejected for want of a neighbour's row."""
+    from paper_2606_16747_b200.sharding import band_matrix, extended_band, halo_rows, shard_rows
+    seq = noit_scenes.cfg5(0, W=960, H=540)
+    W, H = seq.width, seq.height
+    ctx = noit.Noit(seq.weights, seq.mlp_precision)
+    f0 = seq.frame(0)
+    prev = ctx.resolve(noit.DeviceFragBuf.from_host(f0), seq.background)
+    M = seq.reproject_matrix(1)
+    whole = ctx.reproject(W, H, M, seq.depth_threshold, seq.background, prev["trans"], prev["depth1"],
+                          prev["depth1"])
+    acc_whole = whole["accept"].cpu().numpy().reshape(H, W)
+    halo = halo_rows(H)
+    p_t, p_d = prev["trans"].reshape(H, W, 4), prev["depth1"].reshape(H, W)
+    for (y0, y1) in shard_rows(f0.offsets, W, H, 3):
+        e0, e1 = extended_band((y0, y1), halo, H)
+        He = e1 - e0
+        Mb = band_matrix(M, H, e0, e1).astype(np.float32)
+        bt = p_t[e0:e1].reshape(-1, 4).contiguous()
+        bd = p_d[e0:e1].reshape(-1).contiguous()
+        got = ctx.reproject(W, He, Mb, seq.depth_threshold, seq.background, bt, bd, bd)
+        ref = oracle.reproject(W, He, Mb, seq.depth_threshold, seq.background, bt.cpu().numpy(),
+                               bd.cpu().numpy(), bd.cpu().numpy())
+        acc = got["accept"].cpu().numpy()
+        assert np.array_equal(acc, ref["accept"])
+        m = acc.astype(bool)
+        assert np.array_equal(got["trans"].cpu().numpy()[m], ref["trans"][m])
+        assert np.array_equal(got["depth"].cpu().numpy()[m], ref["depth"][m])
+        own = acc.reshape(He, W)[y0 - e0:y1 - e0]
+        differ = (own != acc_whole[y0:y1]).mean()
+        assert differ < 2e-3, differ
+        both = (own == 1) & (acc_whole[y0:y1] == 1)
+        a = got["trans"].reshape(He, W, 4)[y0 - e0:y1 - e0].cpu().numpy()[both]
+        b = whole["trans"].reshape(H, W, 4)[y0:y1].cpu().numpy()[both]
+        assert (a == b).all(axis=1).mean() > 0.995
