@@ -162,17 +162,17 @@ quadtree_kernel(const float* __restrict__ image, int W, int H, int metric, uint3
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { s1[c] += q[c]; s2[c] += q[c] * q[c]; }
             }
-            n = __reduce_add_sync(0xffffffffu, n);
+            // n <= 64 and S1_c <= 64 * 255 fit 16-bit fields: 5 warp reductions per cell, not 7
+            const uint32_t pa = __reduce_add_sync(0xffffffffu, s1[0] | (s1[1] << 16));
+            const uint32_t pb = __reduce_add_sync(0xffffffffu, s1[2] | (n << 16));
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                s1[c] = __reduce_add_sync(0xffffffffu, s1[c]);
-                s2[c] = __reduce_add_sync(0xffffffffu, s2[c]);
-            }
+            for (int c = 0; c < 3; ++c) s2[c] = __reduce_add_sync(0xffffffffu, s2[c]);
             if (lane == 0) {
                 Moments m;
-                m.n = n;
+                m.n = pb >> 16;
+                m.s1[0] = pa & 0xffffu; m.s1[1] = pa >> 16; m.s1[2] = pb & 0xffffu;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) { m.s1[c] = s1[c]; m.s2[c] = s2[c]; }
+                for (int c = 0; c < 3; ++c) m.s2[c] = s2[c];
                 cell[warp * 8 + i] = m;
             }
         }
