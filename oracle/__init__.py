@@ -156,6 +156,23 @@ def resolve_global(fb, half, quarter, weights_eff, background, lod2: int, lod3: 
     return out
 
 
+def resolve10(fb, weights931, background, want_features: bool = False) -> dict:
+    """O12 (NEXT-4): the DFAOIT resolve -- ten features from the fragment list, the 931-parameter
+    sigmoid network predicting the whole transparency colour, Eq. 3 composite."""
+    P = fb.width * fb.height
+    out = dict(trans=np.zeros((P, 4), np.float32), final=np.zeros((P, 4), np.float32),
+               depth1=np.zeros(P, np.float32))
+    if want_features:
+        out["features10"] = np.zeros((P, 10), np.float32)
+    bg = np.asarray(background, np.float32)
+    w = _chk(np.ascontiguousarray(weights931, np.float32), np.float32, 931)
+    args = _fb_args(fb) + [C.c_int32(fb.color_fmt), _p(w), _p(bg), _p(out["trans"]), _p(out["final"]),
+                           _p(out["depth1"]), _p(out.get("features10"))]
+    rc = lib().oracle_resolve10(*args)
+    assert rc == 0, rc
+    return out
+
+
 def exact(fb, background) -> dict:
     """O5x: full sort + Porter-Duff over (Eq. 1) + background; and the exact tail composite."""
     P = fb.width * fb.height

@@ -448,6 +448,76 @@ int32_t oracle_resolve(int32_t width, int32_t height, const uint32_t *offsets, c
 }
 
 /* ---------------------------------------------------------------------------------------- */
+/* O12 (NEXT-4, comparison variant): the DFAOIT resolve STAR-NT starts from (Eq. 3) */
+/* ---------------------------------------------------------------------------------------- */
+/* "The original DFAOIT directly predicts the transparency color C_t using 10 input features"
+ * (P:99), composited as C_p = C_t + C_b prod_{i=1..n} (1 - alpha_i) (Eq. 3).  P:104 lists
+ * "the exact Porter-Duff blended color of the two front fragments" (3), "the average color C_avg"
+ * (3) "and average opacity alpha_avg" (1) "of the remaining n-2 fragments", "the accumulated
+ * premultiplied color C_acc" (3) "and the fragment count n" (1): eleven scalars for ten inputs.
+ * Reading A29: the ten network inputs are the ten colour / opacity scalars, in the
+ * paper's order; n is the count the two averages are taken over (n - 2), not an input:
+ *   x[0..2] = alpha1 C1 + (1 - alpha1) alpha2 C2        (layers by O1; "over", premultiplied)
+ *   x[3..5] = (1/m) sum_tail C_i,   x[6] = (1/m) sum_tail alpha_i,   m = max(n - 2, 0)
+ *   x[7..9] = sum_tail alpha_i C_i                       (the same C_acc as O2)
+ * with all tail entries 0 when m = 0.  The network (oracle_infer10's: 10 -> 32 -> 16 -> 3, ReLU
+ * hidden, SIGMOID output) predicts the whole transparency colour C_t for every pixel with
+ * n >= 1 -- the two exact layers are NOT decoupled, which is the limitation P:106 names; an
+ * empty pixel (n = 0) has C_t = 0 (nothing to predict; the paper is silent).  T_tot is the
+ * product over ALL fragments in index order.  Parity with the DFAOIT authors' feature order and
+ * scaling: unpinned (their paper and code are not in the container).                          */
+static void features10_from(const frag_view *fb, const pixel_layers *L, size_t p, float x[10],
+                            double *t_all)
+{
+    uint32_t b = fb->offsets[p], e = fb->offsets[p + 1];
+    double sum_c[3] = {0, 0, 0}, sum_a = 0.0, t = 1.0;
+    uint32_t m = 0;
+    for (uint32_t j = b; j < e; ++j) {
+        double c[4];
+        frag_rgba(fb, j, c);
+        t *= (1.0 - c[3]);                           /* prod over all n fragments (Eq. 3)     */
+        if (j == L->i1 || j == L->i2) continue;
+        for (int k = 0; k < 3; ++k) sum_c[k] += c[k];
+        sum_a += c[3];
+        ++m;
+    }
+    double a1 = L->c1[3], a2 = L->c2[3];
+    for (int k = 0; k < 3; ++k) {
+        x[k] = (float)(a1 * L->c1[k] + (1.0 - a1) * a2 * L->c2[k]);
+        x[3 + k] = m ? (float)(sum_c[k] / (double)m) : 0.0f;
+        x[7 + k] = (float)L->c_acc[k];
+    }
+    x[6] = m ? (float)(sum_a / (double)m) : 0.0f;
+    *t_all = t;
+}
+
+/* w931 as in oracle_infer10.  Outputs as oracle_resolve; features10 [P][10] optional.         */
+int32_t oracle_resolve10(int32_t width, int32_t height, const uint32_t *offsets, const float *depth,
+                         const void *rgba, int32_t color_fmt, const float *w931,
+                         const float *background, float *out_trans, float *out_final,
+                         float *out_depth1, float *features10)
+{
+    if (!offsets || !w931 || !background) return 1;
+    frag_view fb = {width, height, offsets, depth, rgba, color_fmt};
+    int64_t P = (int64_t)width * height;
+#pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t p = 0; p < P; ++p) {
+        pixel_layers L;
+        float x[10], rgb[3];
+        double t_all, ct[3] = {0, 0, 0};
+        pixel_select_reduce(&fb, (size_t)p, &L);
+        features10_from(&fb, &L, (size_t)p, x, &t_all);
+        if (features10) memcpy(features10 + 10 * p, x, sizeof x);
+        if (L.n > 0) {
+            oracle_infer10(w931, x, 1, rgb);
+            for (int k = 0; k < 3; ++k) ct[k] = (double)rgb[k];
+        }
+        store_outputs(p, ct, t_all, background, L.d1, out_trans, out_final, out_depth1);
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------- */
 /* O5x exact reference: sort every fragment (O1 order), then Eq. 1 read with            */
 /* premultiplied C_p = alpha_p * C_p (A8) plus the background term of Eq. 3.           */
 /* Used by the invariants only.                                                              */

@@ -1241,3 +1241,96 @@ def test_per_pixel_background_closed_form():
     const = np.tile(np.asarray([[0.2, 0.3, 0.4, 0.0]], np.float32), (W * H, 1))
     same = oracle.resolve(fb, w, (0, 0, 0), background_image=const)
     assert np.array_equal(same["final"], ref["final"])
+
+
+# -------------------------------------------------------------------------------------------
+# O12 (NEXT-4): the DFAOIT resolve -- ten features from the fragment list, Eq. 3 composite
+# (reading A29: the ten inputs are the ten colour / opacity scalars of P:104)
+# -------------------------------------------------------------------------------------------
+def _tiny_fb(rng, P, max_n, dtype=np.float32, ties=True):
+    counts = rng.integers(0, max_n + 1, P)
+    off = np.zeros(P + 1, np.uint32)
+    off[1:] = np.cumsum(counts)
+    F = int(off[-1])
+    depth = rng.uniform(0.05, 0.95, F).astype(np.float32)
+    if ties:
+        t = rng.random(F) < 0.4
+        depth[t] = rng.choice(np.asarray([0.25, 0.5], np.float32), int(t.sum()))
+    return FragBuf(P, 1, off, depth, rng.uniform(0, 1, (F, 4)).astype(dtype))
+
+
+def test_features10_against_a_numpy_restatement():
+    """Independent float64 restatement: sort every pixel's fragments by (depth, index) with
+    numpy.lexsort, blend the two nearest with the Porter-Duff "over" operator, average the rest."""
+    rng = np.random.default_rng(60)
+    for dtype in (np.float32, np.float16):
+        fb = _tiny_fb(rng, 400, 9, dtype)
+        got = oracle.resolve10(fb, _weights931(1), BG, want_features=True)["features10"]
+        off = fb.offsets.astype(np.int64)
+        for p in range(fb.num_pixels):
+            d = fb.depth[off[p]:off[p + 1]]
+            c = fb.rgba[off[p]:off[p + 1]].astype(np.float64)
+            order = np.lexsort((np.arange(d.size), d))
+            front, tail = c[order[:2]], c[np.sort(order[2:])]
+            blend = np.zeros(3)
+            for f in front[::-1]:                                    # back to front: C <- a C_f + (1 - a) C
+                blend = f[3] * f[:3] + (1.0 - f[3]) * blend
+            want = np.zeros(10)
+            want[:3] = blend
+            if tail.shape[0]:
+                want[3:6] = tail[:, :3].mean(axis=0)
+                want[6] = tail[:, 3].mean()
+                want[7:10] = (tail[:, 3:4] * tail[:, :3]).sum(axis=0)
+            assert close(got[p], want, 1e-6, 1e-7), (p, got[p], want)
+
+
+def test_features10_closed_forms():
+    rng = np.random.default_rng(61)
+    # uniform tail: every tail fragment has colour c and opacity a => C_avg = c, alpha_avg = a,
+    # C_acc = m a c; the two front fragments are the two smallest depths wherever they sit
+    P, n = 64, 7
+    off = (np.arange(P + 1) * n).astype(np.uint32)
+    depth = rng.uniform(0.3, 0.9, P * n).astype(np.float32)
+    rgba = np.tile(np.asarray([0.25, 0.5, 0.75, 0.125], np.float32), (P * n, 1))
+    for p in range(P):
+        j = rng.choice(n, 2, replace=False) + p * n
+        depth[j] = np.asarray([0.1, 0.2], np.float32)
+        rgba[j] = rng.random((2, 4)).astype(np.float32)
+    x = oracle.resolve10(FragBuf(P, 1, off, depth, rgba), _weights931(0), BG, want_features=True)["features10"]
+    assert np.array_equal(x[:, 3:7], np.tile(np.asarray([0.25, 0.5, 0.75, 0.125], np.float32), (P, 1)))
+    assert close(x[:, 7:10], 5 * 0.125 * np.asarray([0.25, 0.5, 0.75]), 1e-6, 0)
+    # n <= 2: the blend IS the exact composite without a background; no tail entries
+    fb = _tiny_fb(rng, 300, 2)
+    x = oracle.resolve10(fb, _weights931(0), BG, want_features=True)["features10"]
+    assert close(x[:, :3], oracle.exact(fb, (0.0, 0.0, 0.0))["final"][:, :3], 1e-6, 1e-7)
+    assert not x[:, 3:].any()
+    # C_acc is O2's accumulator (already pinned by the tail identities)
+    fb = _tiny_fb(rng, 300, 12, np.float16)
+    x = oracle.resolve10(fb, _weights931(0), BG, want_features=True)["features10"]
+    assert close(x[:, 7:10], oracle.build_features(fb)["tail_raw"][:, :3], 1e-6, 1e-7)
+
+
+def test_resolve10_eq3_structure():
+    """Eq. 3 with a network that outputs a known constant: W3 = 0 and b3 = logit(c) give
+    C_t = c for every non-empty pixel, so C_p = c + C_b prod (1 - alpha_i) and T_tot = the product
+    over ALL fragments (numpy float64 products); empty pixels give (0, 0, 0, 1) and C_p = C_b."""
+    rng = np.random.default_rng(62)
+    fb = _tiny_fb(rng, 500, 10, np.float32)
+    w = _weights931(4)
+    c = np.asarray([0.2, 0.6, 0.9])
+    w[880:928] = 0.0
+    w[928:931] = np.log(c / (1 - c)).astype(np.float32)
+    r = oracle.resolve10(fb, w, BG)
+    off = fb.offsets.astype(np.int64)
+    n = np.diff(off)
+    T = np.asarray([np.prod(1.0 - fb.rgba[off[p]:off[p + 1], 3].astype(np.float64)) for p in range(500)])
+    ct = np.where(n[:, None] > 0, c[None, :], 0.0)
+    assert close(r["trans"][:, :3], ct, 1e-6, 1e-7) and close(r["trans"][:, 3], T, 1e-6, 1e-7)
+    assert close(r["final"][:, :3], ct + T[:, None] * np.asarray(BG), 1e-6, 1e-7)
+    assert close(r["final"][:, 3], 1.0 - T, 1e-6, 1e-7)
+    assert np.array_equal(r["depth1"], oracle.resolve(fb, oracle.effective_weights(noit_scenes.mlp_weights(0), 0), BG)["depth1"])
+    # the network really sees the ten features: the general case equals infer10 on them
+    w = _weights931(5)
+    r = oracle.resolve10(fb, w, BG, want_features=True)
+    f = oracle.infer10(w, r["features10"])
+    assert np.array_equal(r["trans"][n > 0, :3], f[n > 0])
