@@ -429,6 +429,18 @@ def run_ours(args):
               "inference_time_saved_by_5_features": 1.0 - t5 / t10,
               "quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
               "quadtree_balance": timed(lambda: ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal))}
+    # NEXT-4 (O12): the whole DFAOIT resolve (ten features built in the same scan, sigmoid network,
+    # Eq. 3) against the 5-feature resolve with the same FFMA2 network form (fp32 weights) and
+    # against the product path (bf16-rounded weights, tensor-core network): the resolve-level
+    # counterpart of the paper's "10 -> 5 features: 35 % faster inference"
+    ctx32 = noit.Noit(sc.weights, noit.MLP_FP32)
+    outs10 = dict(trans=plain["trans"], final=plain["final"], depth1=plain["depth1"])
+    t10r = timed(lambda: ctx.resolve_dfaoit(fb, w931, BG, want=(), out=outs10))
+    t5f = timed(lambda: ctx32.resolve_desc(d_plain))
+    t5m = timed(lambda: ctx.resolve_desc(d_plain))
+    extras.update({"resolve_dfaoit_10_features_ffma2": t10r, "resolve_5_features_ffma2": t5f,
+                   "resolve_5_features_mma": t5m, "resolve_time_saved_by_5_features_same_network_form": 1.0 - t5f / t10r,
+                   "resolve_time_saved_by_5_features_product_path": 1.0 - t5m / t10r})
     # NEXT-4 (O8b): the step's reprojection with the bilinear fetch, into buffers of its own
     rpb = {"o": None}
     def run_rp(filt):

@@ -164,6 +164,23 @@ noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* desc, void* str
  * (NOIT_ERR_FORMAT if they are not monotone within [0, F]).                                    */
 noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* host_desc, void* stream);
 
+/* ---- NEXT-4: the DFAOIT resolve, the method STAR-NT starts from and is compared with (P:99-104,
+ * Eq. 3; O12, reading A29).  Same fragment buffer, same k = 2 selection and tail scan as
+ * noit_resolve (plain, whole frame), but
+ *   x (10)  = [ a1 C1 + (1-a1) a2 C2 (3),  C_avg (3) and alpha_avg (1) of the n-2 tail fragments,
+ *               C_acc = sum_tail a_i C_i (3) ]          (all tail entries 0 when n <= 2)
+ *   C_t     = sigmoid network 10 -> 32 -> 16 -> 3 (931 parameters, host_w as in noit_infer_dfaoit)
+ *             evaluated on x for every pixel with n >= 1; 0 for an empty pixel
+ *   T_tot   = prod over ALL fragments (1 - a_i);  C_p = C_t + T_tot C_b          (Eq. 3)
+ *   out_trans [P][4] = (C_t, T_tot), out_final [P][4] = (C_p, 1 - T_tot), out_depth1 [P] as in
+ *   noit_resolve; features10 [P][10] (optional, 8-byte aligned) receives x.
+ * The two exact layers are NOT decoupled from the prediction (the limitation P:106 names): this
+ * entry point exists to measure the cost of the 10-feature resolve against the 5-feature one
+ * and as the reference point of Eq. 4.  host_w: 931 floats, host memory.               */
+noit_status noit_resolve_dfaoit(noit_ctx* ctx, const noit_fragbuf* fb, const float* host_w, int32_t count,
+                                const float* background /*[3], host*/, float* out_trans, float* out_final,
+                                float* out_depth1, float* features10, void* stream);
+
 /* ---- S6 quadtree split (sizes 64->8 per BASELINE.json cfg4, A13; O6).
  * Base tiles 64x64 anchored at (0,0), Tx = ceil(W/64), Ty = ceil(H/64).  A node at level
  * l < 3 with >= 1 in-image pixel splits iff metric(node) > threshold (strict); evaluated

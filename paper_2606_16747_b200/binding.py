@@ -22,7 +22,7 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
-           "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit",
+           "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit", "noit_resolve_dfaoit",
            "noit_reproject"]
 
 
@@ -213,6 +213,24 @@ class Noit:
             out = torch.empty((n, 3), dtype=torch.float32, device=features.device)
         self._check(self._L.noit_infer_dfaoit(self._ctx, w.ctypes.data_as(C.c_void_p), C.c_int32(w.size),
                                               _ptr(features), C.c_uint32(n), _ptr(out), _stream(stream)))
+        return out
+
+    def resolve_dfaoit(self, fb: "DeviceFragBuf", weights931, background=(0.0, 0.0, 0.0),
+                       want=("trans", "final", "depth1"), out=None, stream=None):
+        """NEXT-4 (O12): the DFAOIT resolve (ten features, Eq. 3).  `want` may include "features10"."""
+        import numpy as np
+        w = np.ascontiguousarray(weights931, np.float32)
+        P, dev = fb.num_pixels, fb.offsets.device
+        out = dict(out) if out else {}
+        shapes = dict(trans=(P, 4), final=(P, 4), depth1=(P,), features10=(P, 10))
+        for k in want:
+            if k not in out:
+                out[k] = torch.empty(shapes[k], dtype=torch.float32, device=dev)
+        fbc = fb.c_struct()
+        bg = (C.c_float * 3)(*background)
+        self._check(self._L.noit_resolve_dfaoit(
+            self._ctx, C.byref(fbc), w.ctypes.data_as(C.c_void_p), C.c_int32(w.size), bg, _ptr(out.get("trans")),
+            _ptr(out.get("final")), _ptr(out.get("depth1")), _ptr(out.get("features10")), _stream(stream)))
         return out
 
     # ---- S1-S5 (+S7, +S9) ---------------------------------------------------------------

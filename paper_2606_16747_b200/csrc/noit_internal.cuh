@@ -35,6 +35,18 @@ struct MlpWeightsT {
 };
 static_assert(sizeof(MlpWeightsT) <= 4096, "fits the classic kernel-parameter space");
 
+// NEXT-4 (comparison variant): the DFAOIT network, input-major and padded for FFMA2
+// (w1t[i][o], w2t[i][o], w3t[i][o] with o padded to 4 in layer 3); 948 floats as a kernel argument
+struct MlpWeights10T {
+    float w1t[10][32];
+    float b1[32];
+    float w2t[32][16];
+    float b2[16];
+    float w3t[16][4];
+    float b3[4];
+};
+static_assert(sizeof(MlpWeights10T) + 512 <= 4096 * 8, "kernel argument space");
+
 #define NOIT_HOST_BANDS 8
 // work counters: [0, 64) small counters of the quadtree / balance / resolve kernels, then the
 // resolve's ticket counters, one per 128-byte line
@@ -222,6 +234,46 @@ __device__ __forceinline__ void mlp_forward_packed(const MlpWeightsT& W, const f
     f[0] = fmaxf(h3[0].x, 0.f);
     f[1] = fmaxf(h3[0].y, 0.f);
     f[2] = fmaxf(h3[1].x, 0.f);
+}
+
+// O12's network with FFMA2 (same structure as mlp_forward_packed): 10 -> 32 -> 16 -> 3, ReLU hidden,
+// SIGMOID output ("differs only in the output activation"); dot products start from the bias
+// and run in input-index order.
+__device__ __forceinline__ void mlp10_forward_packed(const MlpWeights10T& W, const float x[10], float f[3])
+{
+    float2 h1[16], h2[8], h3[2];
+#pragma unroll
+    for (int o = 0; o < 16; ++o) h1[o] = make_float2(W.b1[2 * o], W.b1[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const float2 xi = make_float2(x[i], x[i]);
+#pragma unroll
+        for (int o = 0; o < 16; ++o)
+            h1[o] = fma2(make_float2(W.w1t[i][2 * o], W.w1t[i][2 * o + 1]), xi, h1[o]);
+    }
+#pragma unroll
+    for (int o = 0; o < 8; ++o) h2[o] = make_float2(W.b2[2 * o], W.b2[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float v = fmaxf((i & 1) ? h1[i >> 1].y : h1[i >> 1].x, 0.f);
+        const float2 hi = make_float2(v, v);
+#pragma unroll
+        for (int o = 0; o < 8; ++o)
+            h2[o] = fma2(make_float2(W.w2t[i][2 * o], W.w2t[i][2 * o + 1]), hi, h2[o]);
+    }
+#pragma unroll
+    for (int o = 0; o < 2; ++o) h3[o] = make_float2(W.b3[2 * o], W.b3[2 * o + 1]);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float v = fmaxf((i & 1) ? h2[i >> 1].y : h2[i >> 1].x, 0.f);
+        const float2 hi = make_float2(v, v);
+#pragma unroll
+        for (int o = 0; o < 2; ++o)
+            h3[o] = fma2(make_float2(W.w3t[i][2 * o], W.w3t[i][2 * o + 1]), hi, h3[o]);
+    }
+    f[0] = 1.0f / (1.0f + expf(-h3[0].x));
+    f[1] = 1.0f / (1.0f + expf(-h3[0].y));
+    f[2] = 1.0f / (1.0f + expf(-h3[1].x));
 }
 
 // ---- O4 on the tensor cores (weights exactly representable in TF32, i.e. NOIT_MLP_BF16) --------

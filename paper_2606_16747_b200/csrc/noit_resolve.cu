@@ -7,6 +7,8 @@
 
 noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A, int color_fmt, int mode,
                                        cudaStream_t st);
+noit_status noit_launch_resolve_dfaoit(noit_ctx* ctx, const ResolveArgs& A, int color_fmt,
+                                       const MlpWeights10T& w10, cudaStream_t st);
 
 // S7 pre-pass: G (10 values in 12 floats) of every coarse pixel whose leaf is resolved at that lod (self-contained
 // O1-O2 on the coarse buffer, A19).  Coarse pixels of other leaves are never sampled: skipped.
@@ -325,3 +327,51 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* s
 }
 
 }  // extern "C"
+
+// NEXT-4 (O12): the DFAOIT resolve, the comparison variant of P:99-104
+extern "C" noit_status noit_resolve_dfaoit(noit_ctx* ctx, const noit_fragbuf* fb, const float* host_w,
+                                           int32_t count, const float* background, float* out_trans,
+                                           float* out_final, float* out_depth1, float* features10,
+                                           void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve_dfaoit: ctx is NULL");
+    NOIT_TRY(noit_check_fragbuf(ctx, fb, "noit_resolve_dfaoit"));
+    if (!host_w || !background) return noit_fail(ctx, NOIT_ERR_NULL, "noit_resolve_dfaoit: host_w / background is NULL");
+    if (count != NOIT_DFAOIT_PARAMS)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_resolve_dfaoit: count %d != 931 (P:97-104)", count);
+    if (!out_trans && !out_final && !out_depth1)
+        return noit_fail(ctx, NOIT_ERR_NULL, "noit_resolve_dfaoit: every output is NULL");
+    if (!noit_aligned(out_trans, 16) || !noit_aligned(out_final, 16) || !noit_aligned(features10, 8))
+        return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_resolve_dfaoit: out_trans/out_final need 16-byte, features10 8-byte alignment");
+    // input-major, padded copy of W1[32][10], b1, W2[16][32], b2, W3[3][16], b3 for the FFMA2 network
+    MlpWeights10T w;
+    memset(&w, 0, sizeof w);
+    const float* W1 = host_w, *b1 = W1 + 320, *W2 = b1 + 32, *b2 = W2 + 512, *W3 = b2 + 16, *b3 = W3 + 48;
+    for (int o = 0; o < 32; ++o) {
+        for (int i = 0; i < 10; ++i) w.w1t[i][o] = W1[o * 10 + i];
+        w.b1[o] = b1[o];
+    }
+    for (int o = 0; o < 16; ++o) {
+        for (int i = 0; i < 32; ++i) w.w2t[i][o] = W2[o * 32 + i];
+        w.b2[o] = b2[o];
+    }
+    for (int o = 0; o < 3; ++o) {
+        for (int i = 0; i < 16; ++i) w.w3t[i][o] = W3[o * 16 + i];
+        w.b3[o] = b3[o];
+    }
+    ResolveArgs A;
+    memset(&A, 0, sizeof A);
+    A.W = fb->width;
+    A.H = fb->height;
+    A.P = (uint32_t)A.W * (uint32_t)A.H;
+    A.F = fb->num_fragments;
+    A.offsets = fb->offsets;
+    A.depth = fb->depth;
+    A.rgba = fb->rgba;
+    memcpy(A.bg, background, sizeof A.bg);
+    A.out_trans = out_trans;
+    A.out_final = out_final;
+    A.out_depth1 = out_depth1;
+    A.features10 = features10;
+    return noit_launch_resolve_dfaoit(ctx, A, fb->color_fmt, w, (cudaStream_t)stream);
+}

@@ -14,6 +14,7 @@ struct ResolveArgs {
     float* out_trans;
     float* out_final;
     float* out_depth1;
+    float* features10;             // NEXT-4 (DFAOIT mode): optional [P][10] inspection output
     // S9
     const uint32_t* pixel_list;
     const uint32_t* pixel_count;

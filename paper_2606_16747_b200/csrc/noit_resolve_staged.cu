@@ -111,6 +111,7 @@ template <> struct Color<__half> {
         v.y &= 0x0000FFFFu;
         return v;
     }
+    static __device__ __forceinline__ void zero_all(Packed* slot) { *slot = make_uint2(0u, 0u); }
     // O2's tail sums for one fragment.  sm_100a has mixed-precision fp32 += fp16 * fp16
     // (`fma.rn.f32.f16`, SASS FHFMA, with half-select operands) and fp32 += fp16 (FHADD): the
     // product of two halves is exact in fp32 and the sum is rounded once, i.e. bit for bit what
@@ -137,6 +138,13 @@ template <> struct Color<__half> {
         const float wf = __half2float(__ushort_as_half(w));
         t = fmaf(-wf, t, t);                               // t *= (1 - alpha), one rounding
     }
+    // O12 (DFAOIT features): also the plain colour sums of the tail (three more FHADD)
+    static __device__ __forceinline__ void accumulate_colour(Packed v, float& cr, float& cg, float& cb)
+    {
+        cr = fhadd((unsigned short)(v.x & 0xffffu), cr);
+        cg = fhadd((unsigned short)(v.x >> 16), cg);
+        cb = fhadd((unsigned short)(v.y & 0xffffu), cb);
+    }
 };
 template <> struct Color<float> {
     typedef float4 Packed;
@@ -145,6 +153,11 @@ template <> struct Color<float> {
     static __device__ __forceinline__ float4 unpack(Packed v) { return v; }
     static __device__ __forceinline__ void zero_alpha(Packed* slot) { slot->w = 0.f; }
     static __device__ __forceinline__ Packed zero_alpha_reg(Packed v) { v.w = 0.f; return v; }
+    static __device__ __forceinline__ void zero_all(Packed* slot) { *slot = make_float4(0.f, 0.f, 0.f, 0.f); }
+    static __device__ __forceinline__ void accumulate_colour(Packed c, float& cr, float& cg, float& cb)
+    {
+        cr += c.x; cg += c.y; cb += c.z;
+    }
     static __device__ __forceinline__ void accumulate(Packed c, float& r, float& g, float& b, float& a, float& t)
     {
         r = fmaf(c.w, c.x, r);
@@ -174,10 +187,11 @@ struct Owned {
     float d1;
     uint32_t n;
     float acc_r, acc_g, acc_b, a_tail, t_tail;
+    float sum_r, sum_g, sum_b;            // O12 only: plain colour sums of the tail
 };
 
 struct Top2 { float d1, d2; uint32_t i1, i2; };
-struct Sums { float r, g, b, a, t; };
+struct Sums { float r, g, b, a, t, cr, cg, cb; };
 
 // newcomer at a larger index wins a slot only on a strictly smaller depth (O1 tie rule)
 __device__ __forceinline__ void top2_push(Top2& s, float d, uint32_t pos)
@@ -219,15 +233,19 @@ __device__ __forceinline__ Top2 scan_depths(const float* D, uint32_t first, uint
     return s;
 }
 // pass 2 over the same positions of the staged colours (layers carry alpha 0)
-template <typename ColorT, int S>
+template <typename ColorT, int S, bool kFeat10 = false>
 __device__ __forceinline__ Sums scan_colours(const typename Color<ColorT>::Packed* C, uint32_t first,
                                              uint32_t end)
 {
     typedef typename Color<ColorT>::Packed Packed;
     Sums s;
     s.r = s.g = s.b = s.a = 0.f;
+    s.cr = s.cg = s.cb = 0.f;
     s.t = 1.f;
-    auto acc = [&](Packed raw) { Color<ColorT>::accumulate(raw, s.r, s.g, s.b, s.a, s.t); };
+    auto acc = [&](Packed raw) {
+        Color<ColorT>::accumulate(raw, s.r, s.g, s.b, s.a, s.t);
+        if (kFeat10) Color<ColorT>::accumulate_colour(raw, s.cr, s.cg, s.cb);
+    };
     uint32_t pos = first;
 #pragma unroll 1
     for (; pos + S < end; pos += 2 * S) {
@@ -260,7 +278,7 @@ __device__ __forceinline__ void transposed_merge(Top2 (&s)[L], int q)
         }
     }
 }
-template <int L>
+template <int L, bool kFeat10 = false>
 __device__ __forceinline__ void transposed_sum(Sums (&s)[L], int q)
 {
 #pragma unroll
@@ -276,13 +294,18 @@ __device__ __forceinline__ void transposed_sum(Sums (&s)[L], int q)
             s[r].b = keep.b + __shfl_xor_sync(0xffffffffu, send.b, m);
             s[r].a = keep.a + __shfl_xor_sync(0xffffffffu, send.a, m);
             s[r].t = keep.t * __shfl_xor_sync(0xffffffffu, send.t, m);
+            if (kFeat10) {
+                s[r].cr = keep.cr + __shfl_xor_sync(0xffffffffu, send.cr, m);
+                s[r].cg = keep.cg + __shfl_xor_sync(0xffffffffu, send.cg, m);
+                s[r].cb = keep.cb + __shfl_xor_sync(0xffffffffu, send.cb, m);
+            }
         }
     }
 }
 
 // ---- cold path: a tile with a round too long for the stage (lists far beyond BASELINE.json's
 // 128-fragment cap) reads global memory directly; the two layers are skipped by index in pass 2.
-template <typename ColorT, int L, int kRounds>
+template <typename ColorT, int L, int kRounds, bool kFeat10 = false>
 __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, uint32_t o1,
                                                        const float* __restrict__ depth,
                                                        const typename Color<ColorT>::Packed* __restrict__ rgba)
@@ -293,6 +316,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
     own.c1 = own.c2 = Color<ColorT>::zero();
     own.d1 = 1.0f; own.n = 0;
     own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
+    own.sum_r = own.sum_g = own.sum_b = 0.f;
     for (int r = 0; r < kRounds; ++r) {
         const int px = r * PPR + g;
         const uint32_t b = __shfl_sync(0xffffffffu, o0, px), e = __shfl_sync(0xffffffffu, o1, px);
@@ -310,18 +334,23 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
         for (int m = 1; m < L; m <<= 1)
             top2_merge(s, __shfl_xor_sync(0xffffffffu, s.d1, m), __shfl_xor_sync(0xffffffffu, s.i1, m),
                        __shfl_xor_sync(0xffffffffu, s.d2, m), __shfl_xor_sync(0xffffffffu, s.i2, m));
-        float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f;
+        float ar = 0.f, ag = 0.f, ab = 0.f, at = 0.f, tt = 1.f, cr = 0.f, cg = 0.f, cb = 0.f;
 #pragma unroll 8
         for (uint32_t j = b + q; j < e; j += L) {
             typename Color<ColorT>::Packed raw = __ldg(rgba + j);
-            if (j == s.i1 || j == s.i2) raw = Color<ColorT>::zero_alpha_reg(raw);
+            if (j == s.i1 || j == s.i2) raw = kFeat10 ? Color<ColorT>::zero() : Color<ColorT>::zero_alpha_reg(raw);
             Color<ColorT>::accumulate(raw, ar, ag, ab, at, tt);
+            if (kFeat10) Color<ColorT>::accumulate_colour(raw, cr, cg, cb);
         }
 #pragma unroll
         for (int m = 1; m < L; m <<= 1) {
             ar += __shfl_xor_sync(0xffffffffu, ar, m); ag += __shfl_xor_sync(0xffffffffu, ag, m);
             ab += __shfl_xor_sync(0xffffffffu, ab, m); at += __shfl_xor_sync(0xffffffffu, at, m);
             tt *= __shfl_xor_sync(0xffffffffu, tt, m);
+            if (kFeat10) {
+                cr += __shfl_xor_sync(0xffffffffu, cr, m); cg += __shfl_xor_sync(0xffffffffu, cg, m);
+                cb += __shfl_xor_sync(0xffffffffu, cb, m);
+            }
         }
         if (q == r) {
             own.c1 = s.i1 != NOIT_ABSENT ? __ldg(rgba + s.i1) : Color<ColorT>::zero();
@@ -329,6 +358,7 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
             own.d1 = s.d1;
             own.n = e - b;
             own.acc_r = ar; own.acc_g = ag; own.acc_b = ab; own.a_tail = at; own.t_tail = tt;
+            own.sum_r = cr; own.sum_g = cg; own.sum_b = cb;
         }
     }
     return own;
@@ -337,10 +367,15 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
 // ------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------
-template <typename ColorT, int L, bool kMma, int kMode>
+// WT = MlpWeightsT: the paper's resolve (O1-O5); WT = MlpWeights10T: the DFAOIT resolve it is
+// compared with (O12: ten features, sigmoid network predicting C_t, Eq. 3) -- same scan, three
+// more sums per tail fragment, the two layers zeroed whole in the stage.
+template <typename ColorT, int L, bool kMma, int kMode, typename WT = MlpWeightsT>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, kMode == NOIT_RESOLVE_LIST ? 7 : NOIT_X_CTAS)
-resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ MlpWeightsT W)
+resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_constant__ WT W)
 {
+    constexpr bool kFeat10 = sizeof(WT) == sizeof(MlpWeights10T);
+    static_assert(!kFeat10 || (!kMma && kMode == NOIT_RESOLVE_ALL), "O12 runs on whole frames with the FFMA2 network");
     typedef typename Color<ColorT>::Packed Packed;
     constexpr uint32_t CB = Color<ColorT>::kBytes;
     // per warp; S9 reads global memory directly and allocates no stage (more CTAs per SM)
@@ -578,6 +613,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
         own.c1 = own.c2 = Color<ColorT>::zero();
         own.d1 = 1.0f; own.n = 0;
         own.acc_r = own.acc_g = own.acc_b = own.a_tail = 0.f; own.t_tail = 1.f;
+        own.sum_r = own.sum_g = own.sum_b = 0.f;
         uint32_t px_own = lane;                          // pixel of the tile this lane ends up owning
 
         // inputs of the epilogue
@@ -613,16 +649,19 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                 const Top2 s = scan_depths<1>(sD, first, end);
                 if (s.i1 != NOIT_ABSENT) {
                     own.c1 = sC2[s.i1];
-                    Color<ColorT>::zero_alpha(&sC2[s.i1]);
+                    if (kFeat10) Color<ColorT>::zero_all(&sC2[s.i1]);
+                    else Color<ColorT>::zero_alpha(&sC2[s.i1]);
                 }
                 if (s.i2 != NOIT_ABSENT) {
                     own.c2 = sC2[s.i2];
-                    Color<ColorT>::zero_alpha(&sC2[s.i2]);
+                    if (kFeat10) Color<ColorT>::zero_all(&sC2[s.i2]);
+                    else Color<ColorT>::zero_alpha(&sC2[s.i2]);
                 }
-                const Sums z = scan_colours<ColorT, 1>(sC2, first, end);    // own list only: no sync
+                const Sums z = scan_colours<ColorT, 1, kFeat10>(sC2, first, end);    // own list only: no sync
                 own.d1 = s.d1;
                 own.n = o1 - o0;
                 own.acc_r = z.r; own.acc_g = z.g; own.acc_b = z.b; own.a_tail = z.a; own.t_tail = z.t;
+                own.sum_r = z.cr; own.sum_g = z.cg; own.sum_b = z.cb;
             }
         } else {
             // ---- heavy tile: L lanes per pixel, L rounds of PPR pixels
@@ -631,7 +670,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             uint32_t B[L + 1];                           // fragment bounds of the rounds
             const bool fits = round_bounds(o0, te, B);
             if (!fits) {
-                own = tile_from_global<ColorT, L, L>(lane, o0, o1, A.depth, g_rgba);
+                own = tile_from_global<ColorT, L, L, kFeat10>(lane, o0, o1, A.depth, g_rgba);
             } else {
                 Top2 t2[L];
                 uint32_t first[L], end[L];
@@ -669,23 +708,26 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                         if (q >= r && q < k) {           // owners of the chunk's rounds
                             if (t2[0].i1 != NOIT_ABSENT) {
                                 own.c1 = Cv[t2[0].i1];
-                                Color<ColorT>::zero_alpha(&Cv[t2[0].i1]);
+                                if (kFeat10) Color<ColorT>::zero_all(&Cv[t2[0].i1]);
+                                else Color<ColorT>::zero_alpha(&Cv[t2[0].i1]);
                             }
                             if (t2[0].i2 != NOIT_ABSENT) {
                                 own.c2 = Cv[t2[0].i2];
-                                Color<ColorT>::zero_alpha(&Cv[t2[0].i2]);
+                                if (kFeat10) Color<ColorT>::zero_all(&Cv[t2[0].i2]);
+                                else Color<ColorT>::zero_alpha(&Cv[t2[0].i2]);
                             }
                         }
                         __syncwarp();
                         staged_to = k;
                     }
-                    sm[r] = scan_colours<ColorT, L>(Cv, first[r], end[r]);
+                    sm[r] = scan_colours<ColorT, L, kFeat10>(Cv, first[r], end[r]);
                 }
-                transposed_sum<L>(sm, q);
+                transposed_sum<L, kFeat10>(sm, q);
                 own.d1 = t2[0].d1;
                 own.n = __shfl_sync(0xffffffffu, o1 - o0, (int)px_own);
                 own.acc_r = sm[0].r; own.acc_g = sm[0].g; own.acc_b = sm[0].b;
                 own.a_tail = sm[0].a; own.t_tail = sm[0].t;
+                own.sum_r = sm[0].cr; own.sum_g = sm[0].cg; own.sum_b = sm[0].cb;
             }
         }
         // the stage is free: start the next tile's first fill, then do this tile's MLP
@@ -744,12 +786,46 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                     e_tt = G2[8];
                 }
             }
-            if (kMma) {                                              // all 32 lanes
-                if (kWeightsInSmem) mlp_forward_mma(MmaWeightsSmem{wsm + lane}, scratch, lane, xf, f);
-                else mlp_forward_mma(MmaWeightsReg{wv}, scratch, lane, xf, f);
+            if constexpr (kFeat10) {
+                // O12 (A29): x = [two-layer "over" blend (3), C_avg (3), alpha_avg, C_acc (3)],
+                // averages over the m = max(n - 2, 0) tail fragments; the sigmoid network predicts the
+                // whole transparency colour; Eq. 3: C_p = C_t + C_b prod (1 - alpha_i)
+                const uint32_t m = own.n > 2u ? own.n - 2u : 0u;
+                const float inv_m = m ? 1.0f / (float)m : 0.f;
+                const float t1 = 1.f - e_c1.w;
+                float x10[10];
+                x10[0] = fmaf(t1, e_l2.x, e_c1.w * e_c1.x);
+                x10[1] = fmaf(t1, e_l2.y, e_c1.w * e_c1.y);
+                x10[2] = fmaf(t1, e_l2.z, e_c1.w * e_c1.z);
+                x10[3] = own.sum_r * inv_m; x10[4] = own.sum_g * inv_m; x10[5] = own.sum_b * inv_m;
+                x10[6] = own.a_tail * inv_m;
+                x10[7] = own.acc_r; x10[8] = own.acc_g; x10[9] = own.acc_b;
+                mlp10_forward_packed(W, x10, f);
+                if (p < A.P) {
+                    if (A.features10) {
+#pragma unroll
+                        for (int k = 0; k < 10; k += 2)
+                            *reinterpret_cast<float2*>(A.features10 + 10 * (size_t)p + k) = make_float2(x10[k], x10[k + 1]);
+                    }
+                    const float keep = own.n ? 1.f : 0.f;            // an empty pixel has no transparency colour
+                    const float ct_r = keep * f[0], ct_g = keep * f[1], ct_b = keep * f[2];
+                    const float t_tot = t1 * (1.f - e_l2.w) * e_tt;
+                    if (A.out_trans)
+                        __stcs(reinterpret_cast<float4*>(A.out_trans) + p, make_float4(ct_r, ct_g, ct_b, t_tot));
+                    if (A.out_final)
+                        __stcs(reinterpret_cast<float4*>(A.out_final) + p,
+                               make_float4(fmaf(t_tot, A.bg[0], ct_r), fmaf(t_tot, A.bg[1], ct_g),
+                                           fmaf(t_tot, A.bg[2], ct_b), 1.f - t_tot));
+                    if (A.out_depth1) __stcs(A.out_depth1 + p, e_d1);
+                }
+            } else {
+                if (kMma) {                                          // all 32 lanes
+                    if (kWeightsInSmem) mlp_forward_mma(MmaWeightsSmem{wsm + lane}, scratch, lane, xf, f);
+                    else mlp_forward_mma(MmaWeightsReg{wv}, scratch, lane, xf, f);
+                }
+                else mlp_forward_packed(W, xf, f);
+                if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
             }
-            else mlp_forward_packed(W, xf, f);
-            if (p < A.P) composite_store(A, p, e_c1, e_l2, e_d1, has_tail, f, e_tt);
         }
         pix = npix; mixed = nmixed; depth_only = ndepth_only;
         t_cur = t_nxt; o0 = no0; o1 = no1;
@@ -768,27 +844,33 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
     }
 }
 
-template <typename ColorT, int L, bool kMma, int kMode>
-static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st)
+template <typename ColorT, int L, bool kMma, int kMode, typename WT = MlpWeightsT>
+static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t st, const WT* w10 = nullptr)
 {
     const size_t stage = kMode == NOIT_RESOLVE_LIST ? 0 : (size_t)kStageBytesFrame;
     const size_t smem = kWarpsPerCta * stage + kWarpsPerCta * sizeof(uint64_t) +
                         kWarpsPerCta * kScratchFloats * sizeof(float) + (kMma ? kWeightBytes : 0);
-    static bool configured = false;                     // per instantiation
-    if (!configured) {
-        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma, kMode>,
+    // the shared-memory attribute and the occupancy are per device (and per instantiation)
+    static int per_sm_dev[64] = {0};
+    const int dev = ctx->device >= 0 && ctx->device < 64 ? ctx->device : 0;
+    if (per_sm_dev[dev] == 0) {
+        NOIT_CUDA(ctx, cudaFuncSetAttribute(resolve_staged_kernel<ColorT, L, kMma, kMode, WT>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
+        int q = 0;
+        NOIT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                           &q, resolve_staged_kernel<ColorT, L, kMma, kMode, WT>, kWarpsPerCta * 32, smem));
+        per_sm_dev[dev] = q < 1 ? -1 : q;
     }
-    int per_sm = 0;
-    NOIT_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                       &per_sm, resolve_staged_kernel<ColorT, L, kMma, kMode>, kWarpsPerCta * 32, smem));
+    const int per_sm = per_sm_dev[dev];
     if (per_sm < 1) return noit_fail(ctx, NOIT_ERR_CUDA, "resolve_staged_kernel does not fit an SM");
     // S9 reads its tile count on the device: the persistent grid is sized for the machine
     const uint32_t want = kMode == NOIT_RESOLVE_LIST ? 0xFFFFFFFFu
                                                      : (A.num_tiles + kWarpsPerCta - 1) / kWarpsPerCta;
     const uint32_t grid = min((uint32_t)(ctx->num_sms * per_sm), max(want, 1u));
-    resolve_staged_kernel<ColorT, L, kMma, kMode><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
+    if constexpr (sizeof(WT) == sizeof(MlpWeights10T))
+        resolve_staged_kernel<ColorT, L, kMma, kMode, WT><<<grid, kWarpsPerCta * 32, smem, st>>>(A, *w10);
+    else
+        resolve_staged_kernel<ColorT, L, kMma, kMode, WT><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
     ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
@@ -833,4 +915,17 @@ noit_status noit_launch_resolve_staged(noit_ctx* ctx, const ResolveArgs& A0, int
         return f16 ? launch_mode<__half, NOIT_RESOLVE_ALL>(ctx, A, st)
                    : launch_mode<float, NOIT_RESOLVE_ALL>(ctx, A, st);
     }
+}
+
+// NEXT-4 (O12): the DFAOIT resolve of a whole frame -- same kernel, ten-feature epilogue
+noit_status noit_launch_resolve_dfaoit(noit_ctx* ctx, const ResolveArgs& A0, int color_fmt,
+                                       const MlpWeights10T& w10, cudaStream_t st)
+{
+    ResolveArgs A = A0;
+    A.num_tiles = (A.P + 31u) / 32u;
+    A.tile_counter = ctx->d_counters;
+    A.mlp_packed = nullptr;
+    return color_fmt == NOIT_RGBA_F16
+               ? launch_staged<__half, 4, false, NOIT_RESOLVE_ALL, MlpWeights10T>(ctx, A, st, &w10)
+               : launch_staged<float, 4, false, NOIT_RESOLVE_ALL, MlpWeights10T>(ctx, A, st, &w10);
 }

@@ -165,6 +165,43 @@ def test_infer_dfaoit_width(noit):
         noit.Noit().infer_dfaoit(w[:771], torch.from_numpy(x).cuda())
 
 
+@pytest.mark.parametrize("dtype,seed,shape,max_n,heavy", [
+    (np.float16, 41, (130, 33), 40, (5, 700)), (np.float32, 42, (67, 45), 12, None),
+    (np.float16, 43, (96, 5), 150, None), (np.float32, 44, (31, 7), 3, (2, 1500)), (np.float16, 45, (1, 1), 9, None)])
+def test_resolve_dfaoit_random(noit, dtype, seed, shape, max_n, heavy):
+    """NEXT-4 / O12: ten features built in the same scan (light, heavy and cold tiles), sigmoid
+    network, Eq. 3 composite, against the oracle; features at the fp32 bar, colours (sigmoid
+    outputs in (0,1)) at 1e-5 absolute on top of it, depth1 bit-exact."""
+    from test_oracle_pins import _weights931
+    rng = np.random.default_rng(seed)
+    fbh = random_fb(rng, shape[0], shape[1], max_n, dtype, heavy=heavy)
+    w = _weights931(seed)
+    got = noit.Noit().resolve_dfaoit(noit.DeviceFragBuf.from_host(fbh), w, BG,
+                                     want=("trans", "final", "depth1", "features10"))
+    ref = oracle.resolve10(fbh, w, BG, want_features=True)
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    close(got["features10"].cpu().numpy(), ref["features10"])
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=1e-5)
+    n = np.diff(fbh.offsets.astype(np.int64))
+    assert not got["trans"].cpu().numpy()[n == 0, :3].any()            # empty pixels: C_t = 0
+
+
+def test_resolve_dfaoit_cfg3_full(noit, cfg3_scene):
+    from test_oracle_pins import _weights931
+    sc = cfg3_scene
+    w = _weights931(3)
+    ctx = noit.Noit()
+    got = ctx.resolve_dfaoit(noit.DeviceFragBuf.from_host(sc.full), w, BG, want=("trans", "final", "depth1", "features10"))
+    ref = oracle.resolve10(sc.full, w, BG, want_features=True)
+    assert np.array_equal(got["depth1"].cpu().numpy(), ref["depth1"])
+    close(got["features10"].cpu().numpy(), ref["features10"])
+    for k in ("trans", "final"):
+        close(got[k].cpu().numpy(), ref[k], extra=1e-5)
+    with pytest.raises(noit.NoitError):
+        ctx.resolve_dfaoit(noit.DeviceFragBuf.from_host(sc.full), w[:771], BG)
+
+
 # -------------------------------------------------------------------------------------------
 # S1-S5 fused
 # -------------------------------------------------------------------------------------------
