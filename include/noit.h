@@ -14,9 +14,20 @@
  *  - Every entry point returns noit_status.  Host-checkable errors (NULL pointers, bad sizes,
  *    unknown enums, missing weights, misalignment) are detected BEFORE any launch and leave all
  *    outputs untouched.  CUDA errors map to NOIT_ERR_CUDA with text in noit_last_error().
- *  - Device-side preconditions are documented, not checked: offsets non-decreasing with
- *    offsets[P] == num_fragments; depth finite; alpha in [0,1]; inputs and outputs do not alias
- *    (except noit_reproject's cur_depth == prev_depth, which is allowed).
+ *  - Device-side preconditions are documented, not checked by the hot entry points: offsets
+ *    non-decreasing with offsets[0] == 0 and offsets[P] == num_fragments (a malformed CSR drives
+ *    the bulk copies out of bounds -- noit_validate_fragbuf checks it on demand); depth finite;
+ *    alpha in [0,1]; inputs and outputs do not alias (except noit_reproject's cur_depth ==
+ *    prev_depth, which is allowed).
+ *  - A context belongs to the device that was current at noit_create; calling a launching entry
+ *    point with another device current is NOIT_ERR_CUDA (nothing is launched).
+ *  - Allocation and synchronisation: entry points never allocate caller-visible memory.  Context
+ *    scratch is allocated with cudaMalloc the FIRST time a call needs it and when a later call
+ *    needs more (noit_resolve with cell_level / pass_scales: G buffers and the tile summary;
+ *    noit_quadtree_balance: one word per tile; noit_resolve_host: the staging area, two streams
+ *    and their events); growing a scratch buffer first synchronises `stream`.  Steady-state calls
+ *    (same sizes) neither allocate nor synchronise, and can be captured in a CUDA graph after one
+ *    eager call.  noit_resolve_host and noit_validate_fragbuf synchronise by definition.
  *  - A context is not thread-safe; distinct contexts are independent.  Calls on ONE context must
  *    be stream-ordered with respect to each other (same stream, or ordered by events): the
  *    context owns small device scratch (work counters, S7 intermediates) that launches share.
@@ -65,6 +76,12 @@ typedef struct {
     const float* depth;            /* [F]                                                     */
     const void* rgba;              /* [F][4]                                                  */
 } noit_fragbuf;
+
+/* Optional check of the device-side CSR preconditions (not on the hot path): offsets[0] == 0,
+ * offsets non-decreasing, offsets[P] == num_fragments.  Runs a small kernel on `stream`,
+ * synchronises it and returns NOIT_OK, or NOIT_ERR_FORMAT with the first offending pixel in
+ * noit_last_error.  Pointers as in every noit_fragbuf: device memory.                        */
+noit_status noit_validate_fragbuf(noit_ctx* ctx, const noit_fragbuf* fb, void* stream);
 
 /* ---- context ------------------------------------------------------------------------------ */
 noit_status noit_create(noit_ctx** out);

@@ -23,6 +23,7 @@ EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights"
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
            "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit", "noit_resolve_dfaoit",
+           "noit_validate_fragbuf",
            "noit_reproject"]
 
 
@@ -177,6 +178,12 @@ class Noit:
     @property
     def launch_count(self) -> int:
         return int(self._L.noit_launch_count(self._ctx))
+
+    def validate_fragbuf(self, fb: "DeviceFragBuf", stream=None):
+        """Raises NoitError(NOIT_ERR_FORMAT) unless offsets are a CSR of fb.num_fragments fragments."""
+        assert fb.offsets.device.index == torch.cuda.current_device(), "fragment buffer on another device"
+        fbc = fb.c_struct()
+        self._check(self._L.noit_validate_fragbuf(self._ctx, C.byref(fbc), _stream(stream)))
 
     # ---- S1-S3 ------------------------------------------------------------------------
     def build_features(self, fb: DeviceFragBuf, want=("idx1", "idx2", "count", "layer1", "layer2",

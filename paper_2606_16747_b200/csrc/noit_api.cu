@@ -23,6 +23,17 @@ noit_status noit_cuda_check(noit_ctx* ctx, cudaError_t e, const char* what)
     return noit_fail(ctx, NOIT_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+noit_status noit_check_device(noit_ctx* ctx, const char* who)
+{
+    int dev = -1;
+    const cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return noit_cuda_check(ctx, e, "cudaGetDevice");
+    if (dev != ctx->device)
+        return noit_fail(ctx, NOIT_ERR_CUDA, "%s: the context was created on device %d, the current device is %d",
+                         who, ctx->device, dev);
+    return NOIT_OK;
+}
+
 noit_status noit_check_fragbuf(noit_ctx* ctx, const noit_fragbuf* fb, const char* name)
 {
     if (!fb) return noit_fail(ctx, NOIT_ERR_NULL, "%s: fragment buffer is NULL", name);

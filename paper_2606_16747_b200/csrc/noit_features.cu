@@ -101,6 +101,7 @@ noit_status noit_infer_dfaoit(noit_ctx* ctx, const float* host_w, int32_t count,
                               uint32_t n, float* rgb, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_infer_dfaoit: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_infer_dfaoit"));
     if (!host_w) return noit_fail(ctx, NOIT_ERR_NULL, "noit_infer_dfaoit: host_w is NULL");
     if (count != NOIT_DFAOIT_PARAMS)
         return noit_fail(ctx, NOIT_ERR_SIZE, "noit_infer_dfaoit: count %d != 931 (P:97-104)", count);
@@ -118,6 +119,7 @@ noit_status noit_build_features(noit_ctx* ctx, const noit_fragbuf* fb, const noi
                                 void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_build_features: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_build_features"));
     NOIT_TRY(noit_check_fragbuf(ctx, fb, "noit_build_features"));
     if (!out) return noit_fail(ctx, NOIT_ERR_NULL, "noit_build_features: out is NULL");
     if (!out->idx1 && !out->idx2 && !out->count && !out->layer1 && !out->layer2 && !out->depth1 &&
@@ -143,6 +145,7 @@ noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* 
                        void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_infer: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_infer"));
     if (!ctx->has_weights) return noit_fail(ctx, NOIT_ERR_NO_WEIGHTS, "noit_infer: no weights set");
     if (n == 0) return NOIT_OK;
     if (!features || !tail_rgb) return noit_fail(ctx, NOIT_ERR_NULL, "noit_infer: NULL buffer");
@@ -153,3 +156,39 @@ noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* 
 }
 
 }  // extern "C"
+
+// ---- noit_validate_fragbuf: the CSR preconditions the hot kernels rely on ---------------------
+__global__ void validate_offsets_kernel(const uint32_t* __restrict__ offsets, uint32_t P, uint32_t F,
+                                        uint32_t* __restrict__ first_bad)
+{
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p > P) return;
+    bool bad = false;
+    if (p == 0) bad = offsets[0] != 0u;
+    if (p == P) bad = bad || offsets[P] != F;
+    if (p < P) bad = bad || offsets[p + 1] < offsets[p];
+    if (bad) atomicMin(first_bad, p);
+}
+
+extern "C" noit_status noit_validate_fragbuf(noit_ctx* ctx, const noit_fragbuf* fb, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_validate_fragbuf: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_validate_fragbuf"));
+    NOIT_TRY(noit_check_fragbuf(ctx, fb, "noit_validate_fragbuf"));
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint32_t P = (uint32_t)fb->width * (uint32_t)fb->height;
+    uint32_t* flag = ctx->d_counters + 20;
+    const uint32_t none = 0xFFFFFFFFu;
+    NOIT_CUDA(ctx, cudaMemcpyAsync(flag, &none, sizeof none, cudaMemcpyHostToDevice, st));
+    validate_offsets_kernel<<<(P + 1 + 255) / 256, 256, 0, st>>>(fb->offsets, P, fb->num_fragments, flag);
+    ctx->launches += 1;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    uint32_t bad = none;
+    NOIT_CUDA(ctx, cudaMemcpyAsync(&bad, flag, sizeof bad, cudaMemcpyDeviceToHost, st));
+    NOIT_CUDA(ctx, cudaStreamSynchronize(st));
+    if (bad != none)
+        return noit_fail(ctx, NOIT_ERR_FORMAT,
+                         "noit_validate_fragbuf: offsets are not a CSR of %u fragments (first violation at pixel %u)",
+                         fb->num_fragments, bad);
+    return NOIT_OK;
+}

@@ -82,6 +82,8 @@ struct noit_ctx {
 noit_status noit_fail(noit_ctx* ctx, noit_status st, const char* fmt, ...);
 noit_status noit_cuda_check(noit_ctx* ctx, cudaError_t e, const char* what);
 noit_status noit_check_fragbuf(noit_ctx* ctx, const noit_fragbuf* fb, const char* name);
+// a context lives on the device that was current at noit_create; every launching entry point checks it
+noit_status noit_check_device(noit_ctx* ctx, const char* who);
 
 #define NOIT_TRY(expr)                      \
     do {                                    \

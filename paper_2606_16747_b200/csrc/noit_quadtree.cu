@@ -298,6 +298,7 @@ extern "C" noit_status noit_quadtree_temporal(noit_ctx* ctx, const float* image,
                                               uint8_t* cell_level, uint32_t* level_hist, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree_temporal: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_quadtree_temporal"));
     if (!image || !params)
         return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_temporal: image/params is NULL");
     if (params->max_level_step < 0 || params->max_level_step > 3)
@@ -318,6 +319,7 @@ extern "C" noit_status noit_quadtree(noit_ctx* ctx, const float* image, int32_t 
                                      uint8_t* cell_level, uint32_t* level_hist, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_quadtree"));
     if (!image || !params) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree: image/params is NULL");
     QtTemporal tq = {nullptr, 0u, 0.f, 0};
     return quadtree_launch(ctx, "noit_quadtree", image, width, height, params->metric,
@@ -414,6 +416,7 @@ extern "C" noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32
                                              void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree_balance: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_quadtree_balance"));
     if (!tile_mask) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance: tile_mask is NULL");
     if (scales && !level_hist)
         return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance: scales needs level_hist");
@@ -547,6 +550,7 @@ extern "C" noit_status noit_quadtree16(noit_ctx* ctx, const float* image, int32_
                                        uint8_t* cell_level, uint32_t* level_hist, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree16: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_quadtree16"));
     if (!image || !params) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree16: image/params is NULL");
     if (!tile_mask && !cell_level && !level_hist)
         return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree16: every output is NULL");

@@ -104,6 +104,7 @@ reproject_kernel(const __grid_constant__ ReprojArgs A)
 extern "C" noit_status noit_reproject(noit_ctx* ctx, const noit_reproject_desc* d, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_reproject: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_reproject"));
     if (!d) return noit_fail(ctx, NOIT_ERR_NULL, "noit_reproject: desc is NULL");
     if (!d->prev_trans || !d->prev_depth || !d->cur_depth || !d->out_trans || !d->reject_count)
         return noit_fail(ctx, NOIT_ERR_NULL, "noit_reproject: a required pointer is NULL");

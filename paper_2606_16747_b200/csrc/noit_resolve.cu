@@ -29,7 +29,7 @@ template <typename ColorT>
 __global__ void __launch_bounds__(kPreBlock)
 coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, uint32_t blocks12, int full_w,
                 const uint8_t* __restrict__ cell_level, uchar4 level_to_lod, uint8_t* __restrict__ tile_lod,
-                uint32_t num_tiles, uint32_t P)
+                uint32_t num_tiles, uint32_t P, const float* __restrict__ pass_scales)
 {
     if (blockIdx.x >= blocks12) {                         // lod summary of tile t (per-tile mode)
         const uint32_t t = (blockIdx.x - blocks12) * blockDim.x + threadIdx.x;
@@ -54,6 +54,12 @@ coarse_g_kernel(CoarseLevel lv1, CoarseLevel lv2, uint32_t blocks1, uint32_t blo
     const int lod = second ? 2 : 1, r = 1 << lod;
     const uint32_t q = (blockIdx.x - (second ? blocks1 : 0u)) * blockDim.x + threadIdx.x;
     if (q >= (uint32_t)lv.cw * (uint32_t)lv.ch) return;
+    if (pass_scales) {                                    // frame-global control (O7g, A27): a coarse
+        const float s2 = __ldg(pass_scales + 1), s3 = __ldg(pass_scales + 2);   // buffer neither pass
+        const int l2 = s2 > 0.70710678f ? 0 : (s2 > 0.35355339f ? 1 : 2);       // uses is not scanned
+        const int l3 = s3 > 0.70710678f ? 0 : (s3 > 0.35355339f ? 1 : 2);
+        if (l2 != lod && l3 != lod) return;
+    }
     const int Y = q / lv.cw, X = q - Y * lv.cw;
     if (cell_level) {                                     // NULL: frame-global lod, every pixel
         const int level = cell_level[(size_t)((Y * r) >> 3) * ((full_w + 7) >> 3) + ((X * r) >> 3)] & 3;
@@ -203,10 +209,10 @@ static noit_status resolve_device(noit_ctx* ctx, const noit_resolve_desc* d, cud
             const uint32_t b12 = blocks[0] + blocks[1];
             if (fmt == NOIT_RGBA_F16)
                 coarse_g_kernel<__half><<<b12 + blocks_s, kPreBlock, 0, st>>>(
-                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
+                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P, d->pass_scales);
             else
                 coarse_g_kernel<float><<<b12 + blocks_s, kPreBlock, 0, st>>>(
-                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P);
+                    lv[0], lv[1], blocks[0], b12, A.W, d->cell_level, l2l, ctx->d_tile_lod, num_tiles, A.P, d->pass_scales);
             ctx->launches += 1;
             NOIT_CUDA(ctx, cudaGetLastError());
         }
@@ -220,6 +226,7 @@ extern "C" {
 noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* d, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_resolve"));
     NOIT_TRY(check_desc(ctx, d, "noit_resolve"));
     return resolve_device(ctx, d, (cudaStream_t)stream);
 }
@@ -227,6 +234,7 @@ noit_status noit_resolve(noit_ctx* ctx, const noit_resolve_desc* d, void* stream
 noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve_host: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_resolve_host"));
     if (h && (h->cell_level || h->pixel_list || h->half || h->quarter || h->pass_scales ||
               h->background_image))
         return noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "noit_resolve_host: plain resolve only");
@@ -266,6 +274,16 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* s
     cudaEvent_t* ev_h2d = ctx->host_ev;
     cudaEvent_t* ev_k = ctx->host_ev + NOIT_HOST_BANDS;
     cudaEvent_t ev_start = ctx->host_ev[2 * NOIT_HOST_BANDS], ev_done = ctx->host_ev[2 * NOIT_HOST_BANDS + 1];
+    // every band boundary is checked BEFORE anything is enqueued: a malformed CSR leaves the
+    // caller's buffers untouched
+    for (size_t p0 = 0; p0 < P; p0 += band_px) {
+        const size_t p1 = std::min(P, p0 + band_px);
+        if (hoff[p1] < hoff[p0] || hoff[p1] > F || (p0 == 0 && hoff[0] != 0))
+            return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_resolve_host: offsets are not a CSR of F fragments");
+    }
+    // From here on copies and kernels are in flight on three streams and target the caller's host
+    // buffers: an error inside the loop must not return before they have drained.
+    const noit_status rc = [&]() -> noit_status {
     // the staging area is reused between calls: the copies start after the caller's earlier work
     NOIT_CUDA(ctx, cudaEventRecord(ev_start, st));
     NOIT_CUDA(ctx, cudaStreamWaitEvent(ctx->h2d_stream, ev_start, 0));
@@ -280,8 +298,6 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* s
     for (size_t p0 = 0; p0 < P; p0 += band_px, ++band) {
         const size_t p1 = std::min(P, p0 + band_px), np = p1 - p0;
         const size_t f0 = hoff[p0], f1 = hoff[p1];
-        if (f1 < f0 || f1 > F)
-            return noit_fail(ctx, NOIT_ERR_FORMAT, "noit_resolve_host: offsets are not a CSR of F fragments");
         NOIT_CUDA(ctx, cudaMemcpyAsync(d_off + p0, hoff + p0, 4 * (np + 1), cudaMemcpyHostToDevice, ctx->h2d_stream));
         if (f1 > f0) {
             NOIT_CUDA(ctx, cudaMemcpyAsync(d_depth + f0, h->full.depth + f0, 4 * (f1 - f0), cudaMemcpyHostToDevice,
@@ -324,6 +340,13 @@ noit_status noit_resolve_host(noit_ctx* ctx, const noit_resolve_desc* h, void* s
     NOIT_CUDA(ctx, cudaStreamWaitEvent(st, ev_done, 0));
     NOIT_CUDA(ctx, cudaStreamSynchronize(st));
     return NOIT_OK;
+    }();
+    if (rc != NOIT_OK) {                                  // drain what was enqueued, keep the first error text
+        cudaStreamSynchronize(ctx->h2d_stream);
+        cudaStreamSynchronize(st);
+        cudaStreamSynchronize(ctx->d2h_stream);
+    }
+    return rc;
 }
 
 }  // extern "C"
@@ -335,6 +358,7 @@ extern "C" noit_status noit_resolve_dfaoit(noit_ctx* ctx, const noit_fragbuf* fb
                                            void* stream)
 {
     if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_resolve_dfaoit: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_resolve_dfaoit"));
     NOIT_TRY(noit_check_fragbuf(ctx, fb, "noit_resolve_dfaoit"));
     if (!host_w || !background) return noit_fail(ctx, NOIT_ERR_NULL, "noit_resolve_dfaoit: host_w / background is NULL");
     if (count != NOIT_DFAOIT_PARAMS)

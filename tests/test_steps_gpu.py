@@ -845,3 +845,36 @@ def test_band_reprojection_with_a_row_halo(noit):
         a = got["trans"].reshape(He, W, 4)[y0 - e0:y1 - e0].cpu().numpy()[both]
         b = whole["trans"].reshape(H, W, 4)[y0:y1].cpu().numpy()[both]
         assert (a == b).all(axis=1).mean() > 0.995
+
+
+def test_validate_fragbuf_and_host_resolve_reject_a_malformed_csr(noit, cfg1_scene):
+    """The hot kernels trust the CSR (documented precondition); noit_validate_fragbuf is the
+    on-demand device check, and noit_resolve_host refuses a malformed CSR before it enqueues
+    anything (outputs untouched)."""
+    sc = cfg1_scene
+    ctx = noit.Noit(sc.weights, sc.mlp_precision)
+    fb = noit.DeviceFragBuf.from_host(sc.full)
+    ctx.validate_fragbuf(fb)                                           # a good buffer passes
+    for mutate in ("swap", "first", "last"):
+        off = sc.full.offsets.copy()
+        if mutate == "swap":
+            k = int(np.argmax(np.diff(off.astype(np.int64)) > 0))
+            off[k + 1] = off[k] - 1 if off[k] > 0 else off[k + 2] + 1   # decreasing step
+            if off[k + 1] >= off[k] and off[k + 1] <= off[k + 2]:
+                off[k + 1] = off[k + 2] + 5
+        elif mutate == "first":
+            off[0] = 1
+        else:
+            off[-1] += 3
+        bad = noit.DeviceFragBuf(fb.width, fb.height, torch.from_numpy(off.view(np.int32)).cuda(), fb.depth, fb.rgba)
+        with pytest.raises(noit.NoitError) as e:
+            ctx.validate_fragbuf(bad)
+        assert e.value.status == 3, mutate                              # NOIT_ERR_FORMAT
+    # host entry point: band boundaries are checked before any copy is enqueued
+    P = sc.full.num_pixels
+    hb = FragBuf(sc.full.width, sc.full.height, sc.full.offsets.copy(), sc.full.depth, sc.full.rgba)
+    hb.offsets[0] = 1                                                  # not a CSR: offsets[0] != 0
+    final = np.full((P, 4), -1.0, np.float32)
+    with pytest.raises(noit.NoitError) as e:
+        ctx.resolve_host(hb, BG, out_final=final)
+    assert e.value.status == 3 and (final == -1.0).all()
