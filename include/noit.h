@@ -96,6 +96,12 @@ noit_status noit_get_weights(const noit_ctx* ctx, float* host_out, int32_t count
 const char* noit_last_error(const noit_ctx* ctx);
 /* number of kernels this context has launched so far (bench.py's gpu_launches).              */
 uint64_t noit_launch_count(const noit_ctx* ctx);
+/* Diagnostics.  libnoit_debug.so is the same library with the staged resolve kernel compiled with
+ * -DNOIT_DEBUG_BOUNDS: every shared-memory range a scan, a layer fetch or a bulk copy touches is
+ * checked against the warp's stage and every fragment range against [0, F), violations are
+ * counted on the device (the access is still made).  This call synchronises the device and
+ * writes the count since noit_create to *host_count; the release build always reports 0.        */
+noit_status noit_debug_bounds_violations(noit_ctx* ctx, uint32_t* host_count);
 
 /* ---- S1-S3: k=2 nearest-layer selection + tail reduction + features
  * Any output pointer may be NULL (skipped); at least one must be set.

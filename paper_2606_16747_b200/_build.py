@@ -33,17 +33,25 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+DEBUG_LIB = os.path.join(HERE, "libnoit_debug.so")     # staged kernel with -DNOIT_DEBUG_BOUNDS
+DEBUG_SRC = "noit_resolve_staged.cu"
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every CUDA translation unit and link libnoit.so.  Returns its path."""
-    if not force and not _stale():
+    """Compile every CUDA translation unit and link libnoit.so -- and libnoit_debug.so, the same
+    objects with the staged resolve kernel compiled with -DNOIT_DEBUG_BOUNDS (own bounds checks;
+    tests/test_steps_gpu.py runs the parity cases through it).  Returns libnoit.so's path."""
+    if not force and not _stale() and os.path.exists(DEBUG_LIB):
         return LIB
     nvcc = _nvcc()
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     procs = []
-    for src in SOURCES:
-        obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        cmd = [nvcc, *COMMON, *PER_FILE.get(src, []), *(["-Xptxas", "-v"] if verbose else []),
+    jobs = [(src, src.replace(".cu", ".o"), []) for src in SOURCES]
+    jobs.append((DEBUG_SRC, DEBUG_SRC.replace(".cu", "_debug.o"), ["-DNOIT_DEBUG_BOUNDS"]))
+    for src, oname, extra in jobs:
+        obj = os.path.join(objdir, oname)
+        cmd = [nvcc, *COMMON, *PER_FILE.get(src, []), *extra, *(["-Xptxas", "-v"] if verbose else []),
                "-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((src, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
     objs = []
@@ -54,8 +62,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if pr.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}")
         objs.append(obj)
-    subprocess.check_call([nvcc, "-shared", "-o", LIB, *objs, "-gencode",
-                           "arch=compute_100a,code=sm_100a", "-lcudart"])
+    link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
+    release = objs[:-1]
+    debug = [objs[-1] if o.endswith(DEBUG_SRC.replace(".cu", ".o")) else o for o in release]
+    subprocess.check_call([*link, "-o", LIB, *release])
+    subprocess.check_call([*link, "-o", DEBUG_LIB, *debug])
     return LIB
 
 

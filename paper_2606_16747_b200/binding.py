@@ -23,7 +23,7 @@ EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights"
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
            "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit", "noit_resolve_dfaoit",
-           "noit_validate_fragbuf",
+           "noit_validate_fragbuf", "noit_debug_bounds_violations",
            "noit_reproject"]
 
 
@@ -96,7 +96,13 @@ def lib():
 
 
 def _ptr(t):
-    return None if t is None else C.c_void_p(t.data_ptr())
+    """Device pointer of a tensor (None stays NULL); a tensor on another device than the current one
+    would be dereferenced by a context of the wrong device: refuse it here."""
+    if t is None:
+        return None
+    if t.is_cuda and t.device.index != torch.cuda.current_device():
+        raise ValueError(f"tensor on cuda:{t.device.index} passed while cuda:{torch.cuda.current_device()} is current")
+    return C.c_void_p(t.data_ptr())
 
 
 def _stream(stream=None):
@@ -174,6 +180,12 @@ class Noit:
         self._check(self._L.noit_get_weights(self._ctx, w.ctypes.data_as(C.c_void_p),
                                              C.c_int32(MLP_PARAMS)))
         return w
+
+    def debug_bounds_violations(self) -> int:
+        """Violations counted by a NOIT_DEBUG_BOUNDS build of the library (0 in the release build)."""
+        n = C.c_uint32(0)
+        self._check(self._L.noit_debug_bounds_violations(self._ctx, C.byref(n)))
+        return int(n.value)
 
     @property
     def launch_count(self) -> int:

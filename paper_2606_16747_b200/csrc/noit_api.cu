@@ -187,4 +187,13 @@ const char* noit_last_error(const noit_ctx* ctx) { return ctx ? ctx->err : g_err
 
 uint64_t noit_launch_count(const noit_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+noit_status noit_debug_bounds_violations(noit_ctx* ctx, uint32_t* host_count)
+{
+    if (!ctx || !host_count) return noit_fail(ctx, NOIT_ERR_NULL, "noit_debug_bounds_violations: NULL argument");
+    NOIT_TRY(noit_check_device(ctx, "noit_debug_bounds_violations"));
+    NOIT_CUDA(ctx, cudaDeviceSynchronize());
+    NOIT_CUDA(ctx, cudaMemcpy(host_count, ctx->d_counters + NOIT_DEBUG_COUNTER, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    return NOIT_OK;
+}
+
 }  // extern "C"

@@ -50,6 +50,7 @@ static_assert(sizeof(MlpWeights10T) + 512 <= 4096 * 8, "kernel argument space");
 #define NOIT_HOST_BANDS 8
 // work counters: [0, 64) small counters of the quadtree / balance / resolve kernels, then the
 // resolve's ticket counters, one per 128-byte line
+#define NOIT_DEBUG_COUNTER 24          // d_counters[24]: violations counted by a NOIT_DEBUG_BOUNDS build
 #define NOIT_TICKET_COUNTERS_LOG2 2
 #define NOIT_COUNTER_WORDS (64 + 32 * (1 << NOIT_TICKET_COUNTERS_LOG2))
 struct noit_ctx {

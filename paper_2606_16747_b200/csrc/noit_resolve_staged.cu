@@ -53,6 +53,27 @@ constexpr uint32_t kScratchFloats = 32 * 12;   // per warp: feature / output tra
 constexpr int kWarpsPerCta = NOIT_X_WARPS;
 constexpr bool kWeightsInSmem = NOIT_X_WSMEM != 0;
 constexpr uint32_t kWeightBytes = kWeightsInSmem ? NOIT_MMA_CHUNKS * 32 * 16 : 0;
+
+// Bounds-checked build (-DNOIT_DEBUG_BOUNDS, libnoit_debug.so; compute-sanitizer is closed on the
+// GPU pool): every range of the warp's stage a scan, a layer fetch or a bulk copy is about to touch
+// is checked against the stage, every global fragment range against [0, F); a violation is counted
+// in a context counter (noit_debug_bounds_violations) and the access is still made, so a parity
+// run of this build that counts zero has made no out-of-stage shared or out-of-range global access.
+#ifdef NOIT_DEBUG_BOUNDS
+#define NOIT_CHK_STAGE(ptr, bytes)                                                                  \
+    do {                                                                                            \
+        const unsigned char* _q = reinterpret_cast<const unsigned char*>(ptr);                     \
+        if ((bytes) != 0 && (_q < stage || _q + (bytes) > stage + kStageBytes))                    \
+            atomicAdd(A.tile_counter + NOIT_DEBUG_COUNTER, 1u);                                     \
+    } while (0)
+#define NOIT_CHK_FRAGS(first, count)                                                                \
+    do {                                                                                            \
+        if ((uint64_t)(first) + (uint64_t)(count) > (uint64_t)A.F) atomicAdd(A.tile_counter + NOIT_DEBUG_COUNTER, 1u); \
+    } while (0)
+#else
+#define NOIT_CHK_STAGE(ptr, bytes) do {} while (0)
+#define NOIT_CHK_FRAGS(first, count) do {} while (0)
+#endif
 constexpr uint32_t kCounterShift = NOIT_TICKET_COUNTERS_LOG2;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
@@ -520,15 +541,17 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             n4 = (A.F - fs) & ~3u;
             const uint32_t rem = fe - fs > n4 ? fe - fs - n4 : 0u;
             if ((uint32_t)lane < rem) {
-                if (has_d) dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane);
-                if (has_c) dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane);
+                NOIT_CHK_FRAGS(fs + n4 + lane, 1u);
+                if (has_d) { NOIT_CHK_STAGE(dst_d + n4 + lane, 4u); dst_d[n4 + lane] = __ldg(A.depth + fs + n4 + lane); }
+                if (has_c) { NOIT_CHK_STAGE(dst_c + n4 + lane, CB); dst_c[n4 + lane] = __ldg(g_rgba + fs + n4 + lane); }
             }
         }
         if (lane == 0 && n4) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(bar, n4 * ((has_d ? 4u : 0u) + (has_c ? CB : 0u)));
-            if (has_d) bulk_g2s(smem_u32(dst_d), A.depth + fs, n4 * 4u, bar);
-            if (has_c) bulk_g2s(smem_u32(dst_c), g_rgba + fs, n4 * CB, bar);
+            NOIT_CHK_FRAGS(fs, n4);
+            if (has_d) { NOIT_CHK_STAGE(dst_d, n4 * 4u); bulk_g2s(smem_u32(dst_d), A.depth + fs, n4 * 4u, bar); }
+            if (has_c) { NOIT_CHK_STAGE(dst_c, n4 * CB); bulk_g2s(smem_u32(dst_c), g_rgba + fs, n4 * CB, bar); }
         }
         pend = n4 != 0;
     };
@@ -636,8 +659,9 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             // staged (4 of the 12 bytes per fragment) and the winner's colour is fetched directly
             if (te > tb) {
                 wait_fill();
+                NOIT_CHK_STAGE(sD + (o0 - fs), (o1 - o0) * 4u);
                 const Top2 s = scan_depths<1>(sD, o0 - fs, o1 - fs);
-                if (s.i1 != NOIT_ABSENT) own.c1 = __ldg(g_rgba + fs + s.i1);
+                if (s.i1 != NOIT_ABSENT) { NOIT_CHK_FRAGS(fs + s.i1, 1u); own.c1 = __ldg(g_rgba + fs + s.i1); }
                 own.d1 = s.d1;
                 own.n = o1 - o0;
             }
@@ -646,13 +670,17 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
             if (te > tb) {
                 wait_fill();                             // issued before the previous tile's MLP
                 const uint32_t first = o0 - fs, end = o1 - fs;
+                NOIT_CHK_STAGE(sD + first, (end - first) * 4u);
+                NOIT_CHK_STAGE(sC2 + first, (end - first) * CB);
                 const Top2 s = scan_depths<1>(sD, first, end);
                 if (s.i1 != NOIT_ABSENT) {
+                    NOIT_CHK_STAGE(sC2 + s.i1, CB);
                     own.c1 = sC2[s.i1];
                     if (kFeat10) Color<ColorT>::zero_all(&sC2[s.i1]);
                     else Color<ColorT>::zero_alpha(&sC2[s.i1]);
                 }
                 if (s.i2 != NOIT_ABSENT) {
+                    NOIT_CHK_STAGE(sC2 + s.i2, CB);
                     own.c2 = sC2[s.i2];
                     if (kFeat10) Color<ColorT>::zero_all(&sC2[s.i2]);
                     else Color<ColorT>::zero_alpha(&sC2[s.i2]);
@@ -690,6 +718,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                     const int px = r * PPR + g;
                     first[r] = __shfl_sync(0xffffffffu, o0, px) + q;
                     end[r] = __shfl_sync(0xffffffffu, o1, px);
+                    if (end[r] > first[r]) NOIT_CHK_STAGE(Dv + first[r], (end[r] - first[r]) * 4u);
                     t2[r] = scan_depths<L>(Dv, first[r], end[r]);
                 }
                 transposed_merge<L>(t2, q);              // t2[0]: this lane's pixel, global indices
@@ -707,11 +736,13 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                         Cv = sC - base;
                         if (q >= r && q < k) {           // owners of the chunk's rounds
                             if (t2[0].i1 != NOIT_ABSENT) {
+                                NOIT_CHK_STAGE(Cv + t2[0].i1, CB);
                                 own.c1 = Cv[t2[0].i1];
                                 if (kFeat10) Color<ColorT>::zero_all(&Cv[t2[0].i1]);
                                 else Color<ColorT>::zero_alpha(&Cv[t2[0].i1]);
                             }
                             if (t2[0].i2 != NOIT_ABSENT) {
+                                NOIT_CHK_STAGE(Cv + t2[0].i2, CB);
                                 own.c2 = Cv[t2[0].i2];
                                 if (kFeat10) Color<ColorT>::zero_all(&Cv[t2[0].i2]);
                                 else Color<ColorT>::zero_alpha(&Cv[t2[0].i2]);
@@ -720,6 +751,7 @@ resolve_staged_kernel(const __grid_constant__ ResolveArgs A, const __grid_consta
                         __syncwarp();
                         staged_to = k;
                     }
+                    if (end[r] > first[r]) NOIT_CHK_STAGE(Cv + first[r], (end[r] - first[r]) * CB);
                     sm[r] = scan_colours<ColorT, L, kFeat10>(Cv, first[r], end[r]);
                 }
                 transposed_sum<L, kFeat10>(sm, q);
@@ -872,7 +904,10 @@ static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream
     else
         resolve_staged_kernel<ColorT, L, kMma, kMode, WT><<<grid, kWarpsPerCta * 32, smem, st>>>(A, ctx->wt);
     ctx->launches += 1;
-    NOIT_CUDA(ctx, cudaGetLastError());
+    const cudaError_t e = cudaGetLastError();
+    // a failed launch may leave the self-re-arming counters armed: zero them for the next call
+    if (e != cudaSuccess) cudaMemsetAsync(ctx->d_counters, 0, NOIT_COUNTER_WORDS * sizeof(uint32_t), st);
+    NOIT_CUDA(ctx, e);
     return NOIT_OK;
 }
 

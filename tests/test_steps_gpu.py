@@ -878,3 +878,23 @@ def test_validate_fragbuf_and_host_resolve_reject_a_malformed_csr(noit, cfg1_sce
     with pytest.raises(noit.NoitError) as e:
         ctx.resolve_host(hb, BG, out_final=final)
     assert e.value.status == 3 and (final == -1.0).all()
+
+
+def test_bounds_checked_build_counts_no_violation(noit):
+    """Our own memcheck (compute-sanitizer is closed on the GPU pool): libnoit_debug.so checks every
+    stage range and fragment range the staged kernel touches; tests/debug_bounds_worker.py drives it
+    through every staging regime against the oracle.  Zero violations, and the counter is shown to
+    be live on a malformed CSR."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    dbg = os.path.join(root, "paper_2606_16747_b200", "libnoit_debug.so")
+    assert os.path.exists(dbg), "libnoit_debug.so missing: run __graft_entry__.build()"
+    out = subprocess.run([sys.executable, os.path.join(root, "tests", "debug_bounds_worker.py")],
+                         capture_output=True, text=True, timeout=900, env=dict(os.environ, NOIT_LIBRARY=dbg))
+    assert out.returncode == 0, out.stderr[-3000:]
+    rec = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert rec["cases"] >= 28 and rec["violations"] == 0, rec
+    assert rec["fired_on_malformed_csr"] > 0, rec
