@@ -70,5 +70,31 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_variant(name: str, defines: list, verbose: bool = False) -> str:
+    """A/B build: libnoit_<name>.so = the release objects with the staged resolve kernel recompiled
+    with the given -D flags (NOIT_X_WARPS, NOIT_X_CTAS, NOIT_X_STAGE, NOIT_X_WSMEM; see
+    noit_resolve_staged.cu).  Select it with NOIT_LIBRARY=<path> (binding.lib) and time it with
+    `python bench.py --config cfgK`: how the occupancy experiments of profiles/r02_resolve.md were run."""
+    build()
+    nvcc = _nvcc()
+    objdir = os.path.join(HERE, "build")
+    obj = os.path.join(objdir, f"noit_resolve_staged_{name}.o")
+    cmd = [nvcc, *COMMON, *defines, *(["-Xptxas", "-v"] if verbose else []), "-c",
+           os.path.join(CSRC, DEBUG_SRC), "-o", obj]
+    out = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)
+    if verbose or out.returncode != 0:
+        sys.stderr.write(out.stdout.decode(errors="replace"))
+    if out.returncode != 0:
+        raise RuntimeError("nvcc failed on the variant")
+    objs = [obj if src == DEBUG_SRC else os.path.join(objdir, src.replace(".cu", ".o")) for src in SOURCES]
+    lib = os.path.join(HERE, f"libnoit_{name}.so")
+    subprocess.check_call([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart", "-o", lib, *objs])
+    return lib
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--variant" in sys.argv:
+        i = sys.argv.index("--variant")
+        print(build_variant(sys.argv[i + 1], [a for a in sys.argv[i + 2:] if a.startswith("-D")], verbose="-v" in sys.argv))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
