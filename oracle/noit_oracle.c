@@ -16,11 +16,17 @@
  * (-ffp-contract=off: nothing fuses unless written as fmaf).  OpenMP only parallelises the
  * outer pixel / tile loops; every pixel is computed by the same scalar code.
  *
- * Pins (tests/test_oracle_*.py): brute-force sort, empty-tail identity, exact-tail identity,
- * closed forms, numpy float64 MLP, quadtree closed forms + big-int brute force, reprojection
- * identity / integer shift.  PARITY UNPINNED: agreement of features O3 (reading A1), of the
- * corner metric's constant and of any threshold with the authors' shader / supplemental
- * material / trained weights -- none of those is available.
+ * Pins (tests/test_oracle_pins.py; every FUNCTION here is pinned against something other than
+ * itself): brute-force sort, empty-tail identity, exact-tail identity, closed forms, numpy float64
+ * MLP, quadtree closed forms + big-int brute force + the quantiser's clamp on out-of-range colours,
+ * adaptive / frame-global identities, reprojection identity / integer shift / threshold flips /
+ * M = s*I (the homogeneous divide) / a dyadic depth row / two cameras against a float64
+ * un-projection, balance closed forms, temporal hysteresis in both threshold orders, the DFAOIT
+ * features against a numpy lexsort restatement and Eq. 3's structure.
+ * PARITY UNPINNED (readings, not functions): agreement of features O3 (reading A1), of the corner
+ * metric's constant, of any threshold, of the trained weights and of the DFAOIT feature order
+ * (reading A29) with the authors' shaders / supplemental material -- none of those is available
+ * (P:55).
  */
 #include <math.h>
 #ifdef _OPENMP
