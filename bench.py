@@ -542,6 +542,10 @@ def run_info(args):
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     name = args.config
+    if name.startswith("synth:"):
+        return run_synth(args, name)
+    if name not in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
+        raise SystemExit(f"bench.py: unknown --config {name}")
     if name == "cfg5":
         seq = noit_scenes.cfg5(0)
         sc = noit_scenes.Scene("cfg5-frame0", seq.frame(0), weights=seq.weights, mlp_precision=seq.mlp_precision)
@@ -602,6 +606,52 @@ def run_info(args):
     print(json.dumps(rec))
 
 
+def run_synth(args, name):
+    """`--config synth:LO-HI`: a 1920x1080 frame whose every pixel holds U{LO..HI} fragments (random
+    depths and fp16 colours drawn on the device): separates the per-pixel cost of the resolve from
+    its per-fragment cost (profiles/r02_resolve.md)."""
+    import torch
+
+    import noit_scenes
+    import paper_2606_16747_b200 as noit
+    lo, hi = (int(v) for v in name.split(":")[1].split("-"))
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    W, H = 1920, 1080
+    P = W * H
+    counts = np.random.default_rng(1).integers(lo, hi + 1, P)
+    off = np.zeros(P + 1, np.uint32)
+    off[1:] = np.cumsum(counts)
+    F = int(off[-1])
+    torch.manual_seed(1)
+    fb = noit.DeviceFragBuf(W, H, torch.from_numpy(off.view(np.int32)).to(dev),
+                            torch.rand(F, device=dev) * 0.98 + 0.01, torch.rand((F, 4), device=dev).half())
+    ctx = noit.Noit(noit_scenes.mlp_weights(0), noit.MLP_BF16)
+    f32 = dict(dtype=torch.float32, device=dev)
+    out = dict(trans=torch.empty((P, 4), **f32), final=torch.empty((P, 4), **f32), depth1=torch.empty(P, **f32))
+    d = ctx.make_resolve_desc(fb, BG, out["trans"], out["final"], out["depth1"])
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        ctx.resolve_desc(d)
+    ms = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        ctx.resolve_desc(d)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+    t = float(np.mean(ms))
+    peak, peak_src = peaks()
+    rbytes = resolve_bytes(P, F, 8, 2, True)
+    print(json.dumps({"info": True, "config": name, "pixels": P, "fragments": F, "fragments_per_tile": F / (P / 32),
+                      "steps": args.steps, "resolve_ms": t, "resolve_gbs": rbytes / t / 1e6,
+                      "resolve_frac_of_hbm_peak": rbytes / t / 1e6 / peak, "peak_source": peak_src,
+                      "memory_floor_ms": rbytes / peak / 1e6}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -613,8 +663,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="time the step eagerly (no CUDA graph)")
     ap.add_argument("--no-fork", action="store_true", help="graph replay of the serial step only")
-    ap.add_argument("--config", default=None, choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"],
-                    help="information only: time one of BASELINE.json's other configs")
+    ap.add_argument("--config", default=None,
+                    help="information only: time the plain resolve of one of BASELINE.json's other configs "
+                         "(cfg1 .. cfg5), or of a synthetic 1080p frame with lo..hi fragments in every pixel "
+                         "(synth:LO-HI): the rate each path of the kernel reaches")
     args = ap.parse_args()
     if os.environ.get("NOIT_BENCH_DRYRUN"):
         return run_dryrun(args)
