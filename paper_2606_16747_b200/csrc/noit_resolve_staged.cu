@@ -48,6 +48,9 @@ namespace {
 #ifndef NOIT_X_WSMEM
 #define NOIT_X_WSMEM 0
 #endif
+#ifndef NOIT_X_PAD
+#define NOIT_X_PAD 0                 // extra dynamic shared memory per CTA: lowers the occupancy, same code
+#endif
 constexpr uint32_t kStageBytesFrame = NOIT_X_STAGE;   // per warp stage (1000 fragments with fp16 colour)
 constexpr uint32_t kScratchFloats = 32 * 12;   // per warp: feature / output transpose of the MMA MLP
 constexpr int kWarpsPerCta = NOIT_X_WARPS;
@@ -881,7 +884,8 @@ static noit_status launch_staged(noit_ctx* ctx, const ResolveArgs& A, cudaStream
 {
     const size_t stage = kMode == NOIT_RESOLVE_LIST ? 0 : (size_t)kStageBytesFrame;
     const size_t smem = kWarpsPerCta * stage + kWarpsPerCta * sizeof(uint64_t) +
-                        kWarpsPerCta * kScratchFloats * sizeof(float) + (kMma ? kWeightBytes : 0);
+                        kWarpsPerCta * kScratchFloats * sizeof(float) + (kMma ? kWeightBytes : 0) +
+                        (kMode == NOIT_RESOLVE_LIST ? 0 : NOIT_X_PAD);
     // the shared-memory attribute and the occupancy are per device (and per instantiation)
     static int per_sm_dev[64] = {0};
     const int dev = ctx->device >= 0 && ctx->device < 64 ? ctx->device : 0;
