@@ -423,9 +423,11 @@ def run_ours(args):
     x5 = torch.rand((P, 5), **f32)
     x10 = torch.rand((P, 10), **f32)
     y3 = torch.empty((P, 3), **f32)
-    t5 = timed(lambda: ctx.infer(x5, out=y3))
+    ctx32 = noit.Noit(sc.weights, noit.MLP_FP32)          # fp32 weights: the FFMA form of the network
+    t5 = timed(lambda: ctx32.infer(x5, out=y3))
+    t5m = timed(lambda: ctx.infer(x5, out=y3))             # bf16-rounded weights: tensor cores
     t10 = timed(lambda: ctx.infer_dfaoit(w931, x10, out=y3))
-    extras = {"infer_5_features": t5, "infer_10_features_dfaoit": t10,
+    extras = {"infer_5_features": t5, "infer_5_features_mma": t5m, "infer_10_features_dfaoit": t10,
               "inference_time_saved_by_5_features": 1.0 - t5 / t10,
               "quadtree_temporal": timed(run_temporal), "quadtree16_corner": timed(run_q16),
               "quadtree_balance": timed(lambda: ctx.quadtree_balance(qt["tile_mask"], W, H, out=bal))}
@@ -433,7 +435,6 @@ def run_ours(args):
     # Eq. 3) against the 5-feature resolve with the same FFMA2 network form (fp32 weights) and
     # against the product path (bf16-rounded weights, tensor-core network): the resolve-level
     # counterpart of the paper's "10 -> 5 features: 35 % faster inference"
-    ctx32 = noit.Noit(sc.weights, noit.MLP_FP32)
     outs10 = dict(trans=plain["trans"], final=plain["final"], depth1=plain["depth1"])
     t10r = timed(lambda: ctx.resolve_dfaoit(fb, w931, BG, want=(), out=outs10))
     t5f = timed(lambda: ctx32.resolve_desc(d_plain))

@@ -50,6 +50,42 @@ infer_kernel(const __grid_constant__ MlpWeights W, const float* __restrict__ fea
     for (int k = 0; k < 3; ++k) tail_rgb[3 * (size_t)r + k] = f[k];
 }
 
+// S4 alone on the tensor cores (bf16-rounded weights, exact in TF32): the two-pass TF32 split of
+// noit_internal.cuh, 32 rows per warp, 8 warps per CTA.  Rows are read and written coalesced
+// through the warp's shared-memory scratch (160 + 96 floats per 32 rows); a grid-stride loop keeps
+// the packed weights (10 float4 per lane) in registers across tiles.
+constexpr int kInferWarps = 8;
+__global__ void __launch_bounds__(kInferWarps * 32)
+infer_mma_kernel(const float4* __restrict__ mlp_packed, const float* __restrict__ features, uint32_t n,
+                 float* __restrict__ tail_rgb)
+{
+    __shared__ __align__(16) float scratch_s[kInferWarps][32 * 12];
+    __shared__ __align__(16) float io_s[kInferWarps][32 * 5];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* const scratch = scratch_s[warp];
+    float* const io = io_s[warp];
+    float4 wv[NOIT_MMA_CHUNKS];
+#pragma unroll
+    for (int v = 0; v < NOIT_MMA_CHUNKS; ++v) wv[v] = __ldg(mlp_packed + v * 32 + lane);
+    const uint32_t tiles = (n + 31u) / 32u, stride = gridDim.x * kInferWarps;
+    for (uint32_t t = blockIdx.x * kInferWarps + warp; t < tiles; t += stride) {
+        const size_t r0 = (size_t)t * 32;
+        const uint32_t rows = min(32u, n - (uint32_t)r0);
+        __syncwarp();
+        for (uint32_t i = lane; i < rows * 5u; i += 32u) io[i] = __ldcs(features + 5 * r0 + i);   // coalesced
+        __syncwarp();
+        float x[5], f[3];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) x[k] = (uint32_t)lane < rows ? io[5 * lane + k] : 0.f;
+        mlp_forward_mma(MmaWeightsReg{wv}, scratch, lane, x, f);
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < 3; ++k) io[3 * lane + k] = f[k];
+        __syncwarp();
+        for (uint32_t i = lane; i < rows * 3u; i += 32u) __stcs(tail_rgb + 3 * r0 + i, io[i]);
+    }
+}
+
 // NEXT-4: the comparison system's network, 10 -> 32 -> 16 -> 3 with a sigmoid output (
 // 931 parameters).  Same shape of kernel as infer_kernel: one row per thread, weights as
 // constant-bank operands of the FFMAs, dot products from the bias in input-index order.
@@ -149,7 +185,14 @@ noit_status noit_infer(noit_ctx* ctx, const float* features, uint32_t n, float* 
     if (!ctx->has_weights) return noit_fail(ctx, NOIT_ERR_NO_WEIGHTS, "noit_infer: no weights set");
     if (n == 0) return NOIT_OK;
     if (!features || !tail_rgb) return noit_fail(ctx, NOIT_ERR_NULL, "noit_infer: NULL buffer");
-    infer_kernel<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(ctx->w, features, n, tail_rgb);
+    if (ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp) {       // weights exact in TF32: tensor cores
+        const uint32_t tiles = (n + 31u) / 32u;
+        const uint32_t grid = min((tiles + kInferWarps - 1) / kInferWarps, (uint32_t)ctx->num_sms * 8u);
+        infer_mma_kernel<<<grid, kInferWarps * 32, 0, (cudaStream_t)stream>>>(
+            static_cast<const float4*>(ctx->d_mlp), features, n, tail_rgb);
+    } else {
+        infer_kernel<<<(n + 127) / 128, 128, 0, (cudaStream_t)stream>>>(ctx->w, features, n, tail_rgb);
+    }
     ctx->launches += 1;
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
