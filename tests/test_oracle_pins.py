@@ -55,6 +55,8 @@ def test_paper_facts():
     assert noit_scenes.mlp_weights(0).shape == (771,)
     # 10-feature DFAOIT net of the same shape would have 931 parameters (context)
     assert 10 * 32 + 32 + 32 * 16 + 16 + 16 * 3 + 3 == 931
+    fl = g["dfaoit_feature_list"]["value"]                     # P:104 lists eleven scalars for ten inputs
+    assert sum(fl.values()) == 11 and sum(fl.values()) - fl["fragment_count_n"] == g["dfaoit_features"]["value"]
     assert g["quadtree_mask_bits"]["value"] == 1 + 4 + 16
     for row in ("Smoke", "Hairball"):                          # Table 1 row sums
         r = g["table1_rows_ms"][row]
