@@ -377,6 +377,32 @@ def test_resolve_cfg3_full_and_layers(noit, cfg3_scene):
     assert sc.meta["tie_pixels"] > 0.05 * sc.full.num_pixels
 
 
+def test_resolve_is_repeatable_over_many_launches(noit, cfg2_scene, cfg3_scene):
+    """Race / scheduling evidence without a race detector: tiles are dealt dynamically (four atomic
+    ticket counters, re-armed by the last warp of each launch), so a lost or doubled ticket, a late
+    counter add, or a race in a warp's stage would show up as an unwritten or differing pixel in
+    SOME launch.  Every launch starts from outputs filled with NaN and must reproduce the first
+    launch bit for bit: 60 launches of cfg2 (all light tiles), 25 of cfg3 (light, heavy, cold)."""
+    for sc, n in ((cfg2_scene, 60), (cfg3_scene, 25)):
+        fb = noit.DeviceFragBuf.from_host(sc.full)
+        ctx = noit.Noit(sc.weights, sc.mlp_precision)
+        P = sc.full.num_pixels
+        out = dict(trans=torch.empty((P, 4), device="cuda"), final=torch.empty((P, 4), device="cuda"),
+                   depth1=torch.empty(P, device="cuda"))
+        d = ctx.make_resolve_desc(fb, BG, out["trans"], out["final"], out["depth1"])
+        ref = None
+        for i in range(n):
+            for t in out.values():
+                t.fill_(float("nan"))
+            ctx.resolve_desc(d)
+            if ref is None:
+                ref = {k: v.clone() for k, v in out.items()}
+                assert not any(torch.isnan(v).any().item() for v in ref.values())
+            else:
+                for k in out:
+                    assert torch.equal(out[k], ref[k]), (sc.name, i, k)
+
+
 def test_resolve_host_matches_device(noit, cfg1_scene):
     sc = cfg1_scene
     ctx = noit.Noit(sc.weights, sc.mlp_precision)
