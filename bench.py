@@ -160,7 +160,7 @@ def max_over_ranks(dist, value: float, device) -> float:
     import torch
     if dist is None:
         return value
-    t = torch.tensor([value], dtype=torch.float64, device=device)
+    t = torch.tensor([value], dtype=torch.float64, device="cpu" if dist.get_backend() == "gloo" else device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
 
@@ -227,9 +227,14 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device and no CPU fallback (use --impl reference for the oracle)")
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # NOIT_BENCH_ONE_GPU=1: functional check of the N > 1 code path on a box with one GPU (every rank on
+    # cuda:0, gloo instead of NCCL, which refuses two ranks on one device) -- its numbers mean nothing
+    one_gpu = bool(os.environ.get("NOIT_BENCH_ONE_GPU"))
+    if one_gpu:
+        local = 0
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    dist, rank, world = dist_setup(args.gpus, "nccl")
+    dist, rank, world = dist_setup(args.gpus, "gloo" if one_gpu else "nccl")
 
     if args.scaling == "strong" and world > 1:
         # strong scaling: ONE cfg3 frame (seed 0) split into 64-row-aligned, fragment-balanced row
