@@ -898,3 +898,37 @@ def test_bounds_checked_build_counts_no_violation(noit):
     rec = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
     assert rec["cases"] >= 28 and rec["violations"] == 0, rec
     assert rec["fired_on_malformed_csr"] > 0, rec
+
+
+def test_one_context_across_frame_sizes(noit):
+    """Context scratch (G buffers, tile summary, balance scratch, counters) grows on demand and is
+    kept between calls: one context driven through a small, a larger and again the small frame --
+    plain, quadtree + balance, adaptive, reproject + pixel list -- must give exactly what fresh
+    contexts give."""
+    scenes = [noit_scenes.cfg4(1, W=192, H=136, n_prims=48, mean_band=(8.0, 10.0), cap=48),
+              noit_scenes.cfg4(2, W=520, H=328, n_prims=96, mean_band=(10.0, 12.0), cap=64)]
+    order = [0, 1, 0, 1]
+    shared = noit.Noit(scenes[0].weights, scenes[0].mlp_precision)
+
+    def run(ctx, sc):
+        fb, hb, qb = (noit.DeviceFragBuf.from_host(b) for b in (sc.full, sc.half, sc.quarter))
+        W, H = fb.width, fb.height
+        plain = ctx.resolve(fb, BG)
+        qt = ctx.quadtree(plain["final"], W, H, 0, 6)
+        bal = ctx.quadtree_balance(qt["tile_mask"].clone(), W, H)
+        ad = ctx.resolve(fb, BG, half=hb, quarter=qb, cell_level=bal["cell_level"])
+        M = np.eye(4, dtype=np.float32)
+        M[0, 3] = 2.0 * 2 / W
+        rp = ctx.reproject(W, H, M, 1e-3, BG, plain["trans"], plain["depth1"], plain["depth1"])
+        out = dict(trans=rp["trans"], final=rp["final"], depth1=rp["depth"])
+        ctx.resolve(fb, BG, out=out, pixel_list=rp["reject_list"], pixel_count=rp["reject_count"])
+        return [plain["final"], plain["trans"], qt["tile_mask"], bal["tile_mask"], bal["cell_level"], bal["hist"],
+                ad["final"], rp["accept"], out["final"], out["trans"]]
+
+    for k in order:
+        sc = scenes[k]
+        shared.set_weights(sc.weights, sc.mlp_precision)
+        got = run(shared, sc)
+        want = run(noit.Noit(sc.weights, sc.mlp_precision), sc)
+        for i, (a, b) in enumerate(zip(got, want)):
+            assert torch.equal(a, b), (k, i)
