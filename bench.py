@@ -474,7 +474,7 @@ def run_ours(args):
                  "balance": "balance_kernel (noit_quadtree_balance, NEXT-1)",
                  "adaptive": "coarse_g_kernel + resolve_staged_kernel<half,4,mma,ADAPTIVE> (noit_resolve, S7)",
                  "reproject": "reproject_kernel<nearest> (noit_reproject, S8)",
-                 "fallback": "resolve_staged_kernel<half,8,ffma2,LIST> (noit_resolve, S9)"}
+                 "fallback": "resolve_staged_kernel<half,2,ffma2,LIST> (noit_resolve, S9)"}
         roofline_all = [{"kernel": kname[k], "step": k, "bytes": int(kb[k]), "ms": per_kernel[k],
                          "achieved_gbs": kb[k] / (per_kernel[k] * 1e-3) / 1e9,
                          "frac": kb[k] / (per_kernel[k] * 1e-3) / 1e9 / peak} for k in names]

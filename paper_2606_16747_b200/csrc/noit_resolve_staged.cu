@@ -48,6 +48,9 @@ namespace {
 #ifndef NOIT_X_WSMEM
 #define NOIT_X_WSMEM 0
 #endif
+#ifndef NOIT_X_LIST_L
+#define NOIT_X_LIST_L 2              // lanes per listed pixel in S9 (32 / L pixels per warp tile)
+#endif
 #ifndef NOIT_X_PAD
 #define NOIT_X_PAD 0                 // extra dynamic shared memory per CTA: lowers the occupancy, same code
 #endif
@@ -921,9 +924,12 @@ static noit_status launch_mode(noit_ctx* ctx, const ResolveArgs& A, cudaStream_t
     // bf16-rounded weights are exact in TF32: the MLP runs on the tensor cores (two-pass split
     // of the activations, fp32-class accuracy); fp32 weights keep the FFMA2 form.
     const bool mma = ctx->precision == NOIT_MLP_BF16 && ctx->d_mlp != nullptr;
-    // lanes per pixel: 4 for frames; 8 for the pixel list (scattered lists are latency-bound:
-    // shorter per-lane chains, 4-pixel tiles keep every warp of the machine busy)
-    constexpr int L = kMode == NOIT_RESOLVE_LIST ? 8 : 4;
+    // lanes per pixel: 4 for frames; 2 for the pixel list (16 listed pixels per warp tile).  Measured on
+    // cfg3 with lists of 0.5 / 1.7 / 5 / 20 % of the pixels (profiles/r02_launches.md): 8 lanes
+    // 18.4 / 31.8 / 56.1 / 163.9 us, 4 lanes 21.0 / 29.7 / 43.2 / 105.4, 2 lanes 23.9 / 25.7 / 41.2 / 91.6,
+    // 1 lane 31.3 / 33.0 / 45.4 / 112.3: with scattered lists the chain offsets -> depths -> colours ->
+    // network is latency, and fewer, fuller tiles mean fewer of those chains per warp.
+    constexpr int L = kMode == NOIT_RESOLVE_LIST ? NOIT_X_LIST_L : 4;
     // S9 is bound by the latency chain of its few scattered tiles, not by issue slots: the FFMA2
     // MLP needs 40 registers fewer than the tensor-core one, which with no stage allocated
     // gives 7 CTAs per SM instead of 4 and so fewer tiles in sequence per warp
