@@ -350,8 +350,11 @@ __device__ __noinline__ Owned<ColorT> tile_from_global(int lane, uint32_t o0, ui
         Top2 s;
         s.d1 = s.d2 = __int_as_float(0x7f800000);
         s.i1 = s.i2 = NOIT_ABSENT;
-        // latency-bound (scattered lists): eight loads in flight per lane, and the colours are
-        // pulled into L2 while the depths are scanned
+        // latency-bound (scattered lists): eight loads in flight per lane; the depth lines of the
+        // whole list are requested into L2 up front (later batches of eight then hit L2), and the
+        // colours are pulled into L2 while the depths are scanned
+        for (uint32_t j = b + 32u * q; j < e; j += 32u * L)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(depth + j));
 #pragma unroll 8
         for (uint32_t j = b + q; j < e; j += L) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(rgba + j));
