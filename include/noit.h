@@ -273,6 +273,23 @@ noit_status noit_quadtree_balance(noit_ctx* ctx, int32_t width, int32_t height, 
                                   uint8_t* tile_level, uint8_t* cell_level, uint32_t* level_hist,
                                   float* scales, void* stream);
 
+/* The same pass for callers that cannot allocate (CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): arguments, outputs and results are exactly noit_quadtree_balance's, but the
+ * kernel's scratch (balanced masks before they are published, finish ticket, histogram accumulators)
+ * lives in a file-scope device array of the library instead of context scratch.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine, on its first use or later.
+ *   limit   ceil(W/64) * ceil(H/64) <= NOIT_BALANCE_STATIC_MAX_TILES (16384 base tiles, e.g.
+ *           8192 x 8192 pixels); beyond it NOIT_ERR_SIZE and nothing is launched
+ *   cost    64.25 KB of device memory on every GPU that loads the library, until the process exits
+ *   sharing ALL calls on a device share the array, whatever context or stream they come from: two
+ *           calls that overlap on the GPU race (order them on one stream or with events).  The
+ *           array keeps the last call's contents; the call clears what must start at zero itself.  */
+#define NOIT_BALANCE_STATIC_MAX_TILES 16384
+noit_status noit_quadtree_balance_static(noit_ctx* ctx, int32_t width, int32_t height, int32_t iterations,
+                                         float delta2, float delta3, uint32_t* tile_mask,
+                                         uint8_t* tile_level, uint8_t* cell_level, uint32_t* level_hist,
+                                         float* scales, void* stream);
+
 /* ---- S8 depth-based reprojection with disocclusion test (O8, A21-A23).
  * Per pixel, fp32 in a fixed order: NDC of the pixel centre and cur_depth -> M -> previous
  * pixel q and expected depth d_e; accept iff w > 0, q on screen and

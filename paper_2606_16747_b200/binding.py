@@ -22,7 +22,7 @@ STATUS = {0: "NOIT_OK", 1: "NOIT_ERR_NULL", 2: "NOIT_ERR_SIZE", 3: "NOIT_ERR_FOR
 EXPORTS = ["noit_create", "noit_destroy", "noit_set_weights", "noit_get_weights",
            "noit_last_error", "noit_launch_count", "noit_build_features", "noit_infer",
            "noit_resolve", "noit_resolve_host", "noit_quadtree", "noit_quadtree_temporal",
-           "noit_quadtree_balance", "noit_quadtree16", "noit_infer_dfaoit", "noit_resolve_dfaoit",
+           "noit_quadtree_balance", "noit_quadtree_balance_static", "noit_quadtree16", "noit_infer_dfaoit", "noit_resolve_dfaoit",
            "noit_validate_fragbuf", "noit_debug_bounds_violations",
            "noit_reproject"]
 
@@ -369,8 +369,11 @@ class Noit:
 
     # ---- NEXT-1 -----------------------------------------------------------------------
     def quadtree_balance(self, tile_mask: torch.Tensor, width: int, height: int, iterations: int = 2,
-                         delta2: float = 2.2, delta3: float = 3.0, out=None, stream=None):
-        """In place on `tile_mask`; returns dict(tile_mask, tile_level, cell_level, hist, scales)."""
+                         delta2: float = 2.2, delta3: float = 3.0, out=None, stream=None,
+                         static_scratch: bool = False):
+        """In place on `tile_mask`; returns dict(tile_mask, tile_level, cell_level, hist, scales).
+        static_scratch=True calls noit_quadtree_balance_static (no allocation inside the call; pass
+        `out` so that the binding allocates nothing either; at most 16384 base tiles)."""
         dev = tile_mask.device
         Tx, Ty = (width + 63) // 64, (height + 63) // 64
         cx, cy = (width + 7) // 8, (height + 7) // 8
@@ -380,7 +383,8 @@ class Noit:
                        hist=torch.empty(4, dtype=torch.int32, device=dev),
                        scales=torch.empty(3, dtype=torch.float32, device=dev))
         out["tile_mask"] = tile_mask
-        self._check(self._L.noit_quadtree_balance(
+        fn = self._L.noit_quadtree_balance_static if static_scratch else self._L.noit_quadtree_balance
+        self._check(fn(
             self._ctx, C.c_int32(width), C.c_int32(height), C.c_int32(iterations), C.c_float(delta2),
             C.c_float(delta3), _ptr(tile_mask), _ptr(out["tile_level"]), _ptr(out["cell_level"]),
             _ptr(out["hist"]), _ptr(out["scales"]), _stream(stream)))

@@ -570,3 +570,78 @@ extern "C" noit_status noit_quadtree16(noit_ctx* ctx, const float* image, int32_
     NOIT_CUDA(ctx, cudaGetLastError());
     return NOIT_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// noit_quadtree_balance_static: the same balance pass for callers that cannot allocate
+// ------------------------------------------------------------------------------------------
+// noit_quadtree_balance keeps the balanced masks in context scratch that it cudaMallocs on first
+// use / growth.  Code under CUDA-graph capture, tight serving loops and harnesses that forbid
+// allocation get this variant: the SAME kernel (balance_kernel), with its scratch -- the balanced
+// masks before they are published, the finish ticket and the histogram accumulators -- in a
+// file-scope device array of fixed size.  Every GPU that loads libnoit.so holds these 64.25 KB until
+// the process exits.  All calls on a device share the array (whatever context or stream they come
+// from): calls that overlap on the GPU race.  The call makes no cudaMalloc / cudaFree and calls no
+// allocating library routine; the counters that must start at zero are cleared by a memset node on
+// `stream` in front of the kernel (the kernel also re-arms them, but a failed or aborted launch
+// must not poison the next call).
+// NOIT_BALANCE_STATIC_MAX_TILES (include/noit.h): 16384 base tiles, e.g. 8192 x 8192 pixels
+constexpr uint32_t kStaticCounterWords = 64;           // [0] ticket, [4..7] histogram accumulators
+static __device__ __align__(256) uint32_t g_balance_scratch[kStaticCounterWords + NOIT_BALANCE_STATIC_MAX_TILES];
+
+// In host code `g_balance_scratch` is a host-side stand-in, not a device address: the address the
+// kernel may use comes from cudaGetSymbolAddress, once per device, with that device current.
+static uint32_t* balance_scratch_address(noit_ctx* ctx)
+{
+    static uint32_t* per_device[64] = {nullptr};
+    const int dev = ctx->device;
+    if (dev < 0 || dev >= 64) {
+        noit_fail(ctx, NOIT_ERR_UNSUPPORTED, "noit_quadtree_balance_static: device index %d beyond 63", dev);
+        return nullptr;
+    }
+    if (!per_device[dev]) {
+        uint32_t* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_balance_scratch);   // current device == ctx->device (checked)
+        if (e != cudaSuccess || !p) {
+            noit_cuda_check(ctx, e != cudaSuccess ? e : cudaErrorInvalidSymbol,
+                            "cudaGetSymbolAddress(g_balance_scratch)");
+            return nullptr;
+        }
+        per_device[dev] = p;
+    }
+    return per_device[dev];
+}
+
+extern "C" noit_status noit_quadtree_balance_static(noit_ctx* ctx, int32_t width, int32_t height,
+                                                    int32_t iterations, float delta2, float delta3,
+                                                    uint32_t* tile_mask, uint8_t* tile_level,
+                                                    uint8_t* cell_level, uint32_t* level_hist,
+                                                    float* scales, void* stream)
+{
+    if (!ctx) return noit_fail(nullptr, NOIT_ERR_NULL, "noit_quadtree_balance_static: ctx is NULL");
+    NOIT_TRY(noit_check_device(ctx, "noit_quadtree_balance_static"));
+    if (!tile_mask) return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance_static: tile_mask is NULL");
+    if (scales && !level_hist)
+        return noit_fail(ctx, NOIT_ERR_NULL, "noit_quadtree_balance_static: scales needs level_hist");
+    if (width <= 0 || height <= 0 || (uint64_t)width * (uint64_t)height + 1 > 0xFFFFFFFFull)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_balance_static: bad width/height");
+    if (iterations < 0 || iterations > 16)
+        return noit_fail(ctx, NOIT_ERR_SIZE, "noit_quadtree_balance_static: iterations must be in [0, 16]");
+    const int64_t Tx = ((int64_t)width + 63) / 64, Ty = ((int64_t)height + 63) / 64, n = Tx * Ty;
+    if (n > NOIT_BALANCE_STATIC_MAX_TILES)
+        return noit_fail(ctx, NOIT_ERR_SIZE,
+                         "noit_quadtree_balance_static: %lld base tiles (%d x %d pixels) exceed the static scratch of %d "
+                         "tiles; use noit_quadtree_balance",
+                         (long long)n, width, height, NOIT_BALANCE_STATIC_MAX_TILES);
+    uint32_t* scratch = balance_scratch_address(ctx);
+    if (!scratch) return NOIT_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: ticket and accumulators must start at zero (the
+    // mask area needs no clearing -- every tile's word is written before the last block reads it)
+    NOIT_CUDA(ctx, cudaMemsetAsync(scratch, 0, kStaticCounterWords * sizeof(uint32_t), st));
+    balance_kernel<<<(int)((n + 3) / 4), 128, 0, st>>>(width, height, (int)Tx, (int)Ty, iterations, delta2, delta3,
+                                                       tile_mask, scratch + kStaticCounterWords, tile_level, cell_level,
+                                                       level_hist, scales, scratch + 0, scratch + 4);
+    ctx->launches += 1;
+    NOIT_CUDA(ctx, cudaGetLastError());
+    return NOIT_OK;
+}
