@@ -891,6 +891,9 @@ def test_bounds_checked_build_counts_no_violation(noit):
     import sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     dbg = os.path.join(root, "paper_2606_16747_b200", "libnoit_debug.so")
+    if not os.path.exists(dbg):                               # a checkout that was never built: build it here
+        from paper_2606_16747_b200 import _build
+        _build.build(force=True)
     assert os.path.exists(dbg), "libnoit_debug.so missing: run __graft_entry__.build()"
     out = subprocess.run([sys.executable, os.path.join(root, "tests", "debug_bounds_worker.py")],
                          capture_output=True, text=True, timeout=900, env=dict(os.environ, NOIT_LIBRARY=dbg))
