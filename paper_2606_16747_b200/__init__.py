@@ -5,5 +5,5 @@ sm_100a).  No CPU fallback: loading fails loudly when the library is missing.
 """
 from .binding import (ABSENT, EXPORTS, MLP_BF16, MLP_FP32, MLP_PARAMS, QT_CORNER, QT_VARIANCE,  # noqa: F401
                       RGBA_F16, RGBA_F32, DeviceFragBuf, Noit, NoitError, lib, lib_path)
-from .sharding import (band_matrix, exchange_halo_rows, extended_band, gather_rows, halo_rows,  # noqa: F401
+from .sharding import (balance_band, band_matrix, exchange_halo_rows, extended_band, gather_rows, halo_rows,  # noqa: F401
                        shard_rows, slice_rows)

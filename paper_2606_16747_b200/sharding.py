@@ -119,3 +119,28 @@ def exchange_halo_rows(band_rows, halo: int, rank: int, world_size: int, group=N
         for w in dist.batch_isend_irecv(ops):
             w.wait()
     return above, below
+
+
+# ---- 2:1 tile balance across bands (NEXT-1): a halo of ORIGINAL masks ------------------------
+def balance_band(ctx, band_mask, width: int, y0: int, y1: int, frame_height: int, above=None, below=None,
+                 iterations: int = 2, delta2: float = 2.2, delta3: float = 3.0):
+    """2:1 balance of one band so that the result equals the whole-frame balance bit for bit.
+
+    k Jacobi steps read ORIGINAL masks within Manhattan distance k, so a band needs
+    its neighbours' nearest k tile rows of original masks ("a 1-tile halo per
+    iteration"): `above` / `below` are those rows ([rows * Tx] int32 tensors, e.g. from
+    exchange_halo_rows on the masks viewed as [tile rows, Tx]; None at the frame edge).  The band is
+    balanced inside the extended strip, then cell levels, histogram and tile levels of its OWN tiles
+    are recomputed with an iterations = 0 call.  Marshalling only: both steps run in balance_kernel.
+    Returns noit.quadtree_balance's dict for the band (the `scales` in it are band-local: the
+    frame's demand index needs the sum of the bands' histograms)."""
+    import torch
+    Tx = (width + TILE - 1) // TILE
+    ra = 0 if above is None else above.numel() // Tx
+    rb = 0 if below is None else below.numel() // Tx
+    parts = [t for t in (above, band_mask, below) if t is not None]
+    ext = torch.cat([p.reshape(-1) for p in parts]).contiguous()
+    ya, yb = y0 - TILE * ra, min(frame_height, y1 + TILE * rb)
+    ctx.quadtree_balance(ext, width, yb - ya, iterations=iterations, delta2=delta2, delta3=delta3)
+    own = ext[ra * Tx: ra * Tx + band_mask.numel()].clone()
+    return ctx.quadtree_balance(own, width, y1 - y0, iterations=0, delta2=delta2, delta3=delta3)

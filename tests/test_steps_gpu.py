@@ -806,6 +806,42 @@ def test_sharded_resolve_and_quadtree_equal_the_whole_frame(noit, world):
         assert abs(frags[0] - frags[1]) < 0.2 * sum(frags)       # balanced by fragments
 
 
+@pytest.mark.parametrize("W,H,cuts", [(1920, 1080, (6, 11)), (3840, 2160, (1, 2, 20)), (640, 1000, (8,))])
+def test_band_balance_with_a_mask_halo_equals_the_whole_frame(noit, W, H, cuts):
+    """NEXT-1 across bands: each band balanced with its neighbours' nearest two tile
+    rows of ORIGINAL masks (the halo exchange_halo_rows would move) equals the whole-frame 2:1
+    balance bit for bit -- masks, tile levels, cell levels -- and the bands' histograms add up to
+    the frame's.  Without the halo a band boundary may break the 2:1 rule (asserted too)."""
+    from test_oracle_pins import _random_valid_masks
+    from paper_2606_16747_b200.sharding import balance_band
+    rng = np.random.default_rng(W + H)
+    Tx, Ty = (W + 63) // 64, (H + 63) // 64
+    m = _random_valid_masks(rng, Tx * Ty)
+    ctx = noit.Noit()
+    whole = ctx.quadtree_balance(torch.from_numpy(m.view(np.int32).copy()).cuda(), W, H)
+    ref = oracle.quadtree_balance(m, W, H)
+    assert np.array_equal(u32(whole["tile_mask"]), ref["tile_mask"])
+    d = torch.from_numpy(m.view(np.int32).copy()).cuda().reshape(Ty, Tx)
+    rows = [0, *cuts, Ty]
+    hist = np.zeros(4, np.int64)
+    differs_without_halo = False
+    cw = (W + 7) // 8
+    for r0, r1 in zip(rows[:-1], rows[1:]):
+        y0, y1 = r0 * 64, min(H, r1 * 64)
+        above = d[max(0, r0 - 2):r0].contiguous() if r0 > 0 else None
+        below = d[r1:min(Ty, r1 + 2)].contiguous() if r1 < Ty else None
+        got = balance_band(ctx, d[r0:r1].contiguous().reshape(-1), W, y0, y1, H, above, below)
+        assert np.array_equal(u32(got["tile_mask"]), ref["tile_mask"][r0 * Tx:r1 * Tx])
+        assert np.array_equal(got["tile_level"].cpu().numpy(), ref["tile_level"][r0 * Tx:r1 * Tx])
+        c0, c1 = (y0 // 8) * cw, ((y1 + 7) // 8) * cw
+        assert np.array_equal(got["cell_level"].cpu().numpy(), ref["cell_level"][c0:c1])
+        hist += u32(got["hist"]).astype(np.int64)
+        alone = balance_band(ctx, d[r0:r1].contiguous().reshape(-1), W, y0, y1, H)
+        differs_without_halo |= not np.array_equal(u32(alone["tile_mask"]), ref["tile_mask"][r0 * Tx:r1 * Tx])
+    assert np.array_equal(hist, ref["hist"].astype(np.int64))
+    assert differs_without_halo or W < 1920                    # the halo is what makes the bands agree
+
+
 def test_band_reprojection_with_a_row_halo(noit):
     """S8 across bands: a band extended by halo_rows(H) rows of its neighbours'
     prev_trans / prev_depth (here: slices of the whole previous frame stand in for the peer copies
