@@ -156,3 +156,23 @@ def test_band_matrix_is_the_frame_matrix_in_band_coordinates():
         rb = (c[1] / c[3] + 1) * 0.5 * (y1 - y0) + y0
         rg = (g[1] / g[3] + 1) * 0.5 * H
         assert abs(rb - rg) < 1e-9 and abs(c[0] / c[3] - g[0] / g[3]) < 1e-12 and abs(c[2] / c[3] - g[2] / g[3]) < 1e-12
+
+
+def test_bench_reference_arm_contract():
+    """`bench.py --impl reference` (the oracle on the host cores): one JSON line with the contract's
+    keys, BASELINE.json's metric string, and a cpu_baseline that describes the run."""
+    import json
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout
+    rec = json.loads(lines[0])
+    want = json.load(open(os.path.join(ROOT, "BASELINE.json")))["metric"]
+    assert rec["impl"] == "reference" and rec["metric"] == want and rec["unit"] == "Mpixels/s"
+    assert rec["value"] > 0 and rec["higher_is_better"] is True and rec["vs_baseline"] is None
+    assert rec["steps"] == 1 and rec["n_gpus"] == 1 and rec["data"] == "synthetic"
+    assert rec["cpu_baseline"]["kind"] == "oracle" and rec["cpu_baseline"]["cores"] >= 1
+    assert rec["cpu_baseline"]["value"] == rec["value"] and rec["cpu_baseline"]["sample"]
+    assert rec["e2e"] == {"value": rec["value"], "unit": "Mpixels/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert rec["config"]["workload"].startswith("cfg3") and rec["gpu_launches"] == 0
